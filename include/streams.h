@@ -1,0 +1,164 @@
+/*
+ * streams.h -- C-ABI boundary of the B200-native STREAmS hot path.
+ *
+ * The library evaluates the explicit right-hand side R(w) of the 3-D compressible
+ * Navier-Stokes equations (Eq. 1-3) on a Cartesian grid that may be
+ * stretched, and advances the conservative state w = [rho, rho u, rho v, rho w, rho E]
+ * with the three-stage low-storage Runge-Kutta scheme of PAPER.md:89-99
+ * (Eq. 10-11).  Everything between `streams_set_state` and `streams_get_state` runs in
+ * hand-written fp64 CUDA kernels for sm_100a on ONE GPU; there is no CPU fallback.
+ *
+ * Conventions
+ *  - Every call returns an int: STREAMS_OK (0) or a negative STREAMS_E* code.  No
+ *    exception crosses the boundary.  `streams_last_error` gives a text for the last
+ *    failure of a context (or of `streams_create` when ctx == NULL).
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The library never
+ *    takes ownership of a caller pointer.  All field arrays are fp64, layout
+ *    [5][nz][ny][nx] (variable slowest, x fastest), NO ghost nodes stored.
+ *  - The library does not allocate field-sized device memory.  The caller (PyTorch in
+ *    this repository) allocates `streams_workspace_bytes()` bytes, 256-byte aligned,
+ *    hands them to `streams_create`, and keeps them alive until `streams_destroy`.
+ *    The context owns only O(nx+ny+nz) metric arrays and a few scalars on the device.
+ *  - All kernels are enqueued on the `cuda_stream` given at creation (a cudaStream_t
+ *    passed as void*, NULL = legacy default stream).  Only `streams_diagnostics`,
+ *    the *_host copies and `streams_destroy` synchronise that stream.
+ *  - Index/ghost convention: nodes 0..n-1 per direction; ghost values (width 3) are
+ *    never stored, they are evaluated by index arithmetic from the boundary kind
+ *    (DESIGN.md "S1").
+ */
+#ifndef STREAMS_H
+#define STREAMS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct streams_ctx streams_ctx; /* opaque; created by streams_create, freed by streams_destroy */
+
+/* error codes */
+enum {
+  STREAMS_OK = 0,
+  STREAMS_EINVAL = -1,     /* bad argument or unsupported combination of parameters   */
+  STREAMS_ECUDA = -2,      /* a CUDA runtime call or kernel launch failed             */
+  STREAMS_ENOMEM = -3,     /* caller workspace too small / misaligned                  */
+  STREAMS_ENONFINITE = -4, /* diagnostics saw NaN/Inf or rho <= 0 or p <= 0            */
+  STREAMS_ESTATE = -5      /* call needs a state but streams_set_state was not called  */
+};
+
+/* boundary kinds, one per face: bc[0..5] = xmin, xmax, ymin, ymax, zmin, zmax */
+enum {
+  STREAMS_BC_PERIODIC = 0,           /* PAPER.md:110, 126 (homogeneous directions)            */
+  STREAMS_BC_WALL_ISO_STAGGERED = 1, /* isothermal no-slip wall half-way between the first two
+                                        nodes, convective flux zero there       */
+  STREAMS_BC_WALL_ISO_NODE = 2,      /* isothermal no-slip wall on the boundary node */
+  STREAMS_BC_INFLOW_FROZEN = 3,      /* Dirichlet ghost planes frozen at set_state (stands in for the
+                                        digital-filter inflow of PAPER.md:126, A16) */
+  STREAMS_BC_OUTFLOW_NR = 4,         /* characteristic non-reflecting boundary   */
+  STREAMS_BC_SHOCKGEN = 5,           /* inviscid oblique-shock state imposed in the ghosts of ymax
+                                                                                 */
+  STREAMS_BC_EXTRAP = 6              /* zeroth-order extrapolation (1-D tube tests)            */
+};
+
+enum { STREAMS_VISC_POWER = 0, STREAMS_VISC_SUTHERLAND = 1 };
+
+/* Grid: node counts and the domain length per direction (the period for periodic
+ * directions; otherwise informational).  Node coordinates are passed to streams_create. */
+typedef struct {
+  int nx, ny, nz;
+  int pad_;
+  double len[3];
+} streams_grid;
+
+/* Gas, scheme, boundary and forcing parameters.  Plain data, copied at creation. */
+typedef struct {
+  double gamma;            /* ratio of specific heats (1.4)                                   */
+  double Pr;               /* Prandtl number (0.72)                              */
+  double Rgas;             /* gas constant in the caller's units: p = rho Rgas T              */
+  double mu_ref, T_ref;    /* viscosity law reference values                                  */
+  double visc_exp;         /* POWER:  mu = mu_ref (T/T_ref)^visc_exp                          */
+  double suth_S;           /* SUTHERLAND: mu = mu_ref (T/T_ref)^1.5 (T_ref+S)/(T+S)           */
+  double sensor_threshold; /* theta_th of the hybrid switch (Eq. 8)              */
+  double sensor_eps;       /* (u0/L0)^2 regulariser of Eq. 8, must be > 0                     */
+  double T_wall[2];        /* wall temperature for the ymin / ymax walls                      */
+  double y_wall[2];        /* wall-plane coordinate for STAGGERED walls (ymin, ymax)          */
+  double fs[5];            /* free-stream primitive state rho,u,v,w,T (SHOCKGEN)              */
+  double shock_angle_deg;  /* flow deflection of the shock generator                          */
+  double x_shock;          /* x at which the jump enters through the ymax ghosts              */
+  double cfl;              /* Courant number for the on-device time step (S10)      */
+  double dt_fixed;         /* > 0: use this time step instead of the CFL reduction            */
+  int visc_model;          /* STREAMS_VISC_*                                                  */
+  int order;               /* 2L: 2, 4 or 6 (6 = measured path)                               */
+  int weno_enable;         /* 1: Ducros-switched WENO5 flux on flagged interfaces             */
+  int forcing;             /* 1: constant bulk mass-flow forcing in x      */
+  int viscous_enable;      /* 0: Euler equations (conservation / KE tests)                    */
+  int bc[6];               /* STREAMS_BC_* for xmin,xmax,ymin,ymax,zmin,zmax                   */
+  int pad_;
+} streams_params;
+
+/* Reductions over the current state (and the last RHS evaluation). */
+typedef struct {
+  long long step;          /* completed RK3 steps                                             */
+  double time, dt, forcing;/* physical time, last time step, last body force f                */
+  double mass, mom[3], energy, kinetic; /* sum over nodes of q * vol, vol = h_x h_y h_z       */
+  double volume;           /* sum of vol                                                      */
+  double bulk_rhou;        /* mom[0] / volume                                                 */
+  double min_rho, min_p, max_mach, max_theta;
+  double max_speed[3];     /* max over nodes of (|u_d| + c) / h_d                             */
+  long long weno_ifaces[3], total_ifaces[3]; /* flagged / total interfaces of the last RHS   */
+  int nonfinite;           /* 1 if NaN/Inf, rho<=0 or p<=0 was seen                           */
+  int pad_;
+} streams_diag;
+
+/* Bytes of device workspace `streams_create` needs for this grid/params (0 on bad input). */
+size_t streams_workspace_bytes(const streams_grid* grid, const streams_params* params);
+
+/* Create a context.  h_x/h_y/h_z: HOST arrays of nx/ny/nz node coordinates, strictly
+ * increasing.  d_workspace: DEVICE memory, >= streams_workspace_bytes(), 256-B aligned,
+ * owned by the caller.  cuda_stream: cudaStream_t as void*.  On success *out is set. */
+int streams_create(const streams_grid* grid, const double* h_x, const double* h_y, const double* h_z,
+                   const streams_params* params, void* d_workspace, size_t workspace_bytes,
+                   void* cuda_stream, streams_ctx** out);
+
+/* Copy a state into the context (device->device, async).  Captures the frozen inflow
+ * plane when bc[xmin] == INFLOW_FROZEN.  Resets step counter, time and RK register. */
+int streams_set_state(streams_ctx* ctx, const double* d_w);
+/* Same from pageable or pinned HOST memory (host->device copy on the context stream; synchronises). */
+int streams_set_state_host(streams_ctx* ctx, const double* h_w);
+
+/* Copy the current state out (device->device, async). */
+int streams_get_state(streams_ctx* ctx, double* d_w_out);
+/* Same into HOST memory (synchronises). */
+int streams_get_state_host(streams_ctx* ctx, double* h_w_out);
+
+/* R(w) of the current state into d_rhs_out ([5][nz][ny][nx]); includes the body force
+ * (forcing=1) and the characteristic replacement at OUTFLOW_NR nodes, excludes the
+ * Dirichlet node overrides of NODE walls.  State, time and step counter unchanged. */
+int streams_rhs(streams_ctx* ctx, double* d_rhs_out);
+
+/* Node flags of the shock sensor for the current state: d_theta_out[nz][ny][nx] fp64
+ * (may be NULL) receives theta of Eq. 8; d_flags_out[3][nz][ny][nx] bytes (may be NULL)
+ * receives 1 where interface i+1/2 (resp. j+1/2, k+1/2) above node (i,j,k) is flagged. */
+int streams_sensor(streams_ctx* ctx, double* d_theta_out, unsigned char* d_flags_out);
+
+/* Advance nsteps full RK3 steps (Eq. 11); dt recomputed on the device every step
+ * unless dt_fixed > 0.  No host synchronisation. */
+int streams_step(streams_ctx* ctx, int nsteps);
+
+/* Reductions of the current state into *h_out (host struct).  Synchronises.  Returns
+ * STREAMS_ENONFINITE (with *h_out filled) if the state is not physical. */
+int streams_diagnostics(streams_ctx* ctx, streams_diag* h_out);
+
+/* Number of kernel launches enqueued by this context so far (for bench accounting). */
+long long streams_launch_count(const streams_ctx* ctx);
+
+/* Text of the last error (never NULL).  ctx may be NULL for streams_create failures. */
+const char* streams_last_error(const streams_ctx* ctx);
+
+void streams_destroy(streams_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STREAMS_H */

@@ -1,0 +1,526 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these tests touches the CUDA path.  Each compares the oracle with something other
+than itself: polynomial exactness, an algebraically different (split) form of the flux,
+conservation / kinetic-energy identities, the textbook Butcher tableau of Wray's RK3, a
+complex-step Jacobian of the Euler flux, the exact Riemann solution, oblique-shock jump
+conditions and sympy-manufactured fields.
+"""
+import math
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from paper_2004_02276_b200 import workloads as W
+from tests import helpers as H
+
+GAM = 1.4
+
+
+@pytest.fixture(scope="module")
+def ob(oracle_mod):
+    return oracle_mod
+
+
+def make(ob, wl):
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    o.set_state(wl.state())
+    return o
+
+
+def line_workload(n, d, params, xs=None, L=1.0):
+    """n nodes along direction d, one (periodic) node along the other two."""
+    nn = [1, 1, 1]
+    nn[d] = n
+    coords = [np.zeros(1), np.zeros(1), np.zeros(1)]
+    coords[d] = xs if xs is not None else L * np.arange(n) / n
+    ln = [1.0, 1.0, 1.0]
+    ln[d] = L
+    grid = dict(nx=nn[0], ny=nn[1], nz=nn[2], len=ln)
+    return grid, coords
+
+
+# ------------------------------------------------------------------ P1: coefficient tables
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_P1_coefficients_polynomial_exactness(ob, order):
+    """a_l, b_l are the standard central coefficients of order 2L.  The oracle's
+    metric routine applies D and D2 to the node coordinates, so coordinates x_i = poly(i) of degree
+    <= 2L must give exactly poly'(i) and poly''(i); degree 2L+1 must show the textbook leading error."""
+    n = 24
+    i = np.arange(n, dtype=float)
+    p = W.default_params(order=order, bc=[W.BC_EXTRAP] * 2 + [W.BC_PERIODIC] * 4)
+    rng = np.random.default_rng(3)
+    c = rng.uniform(0.5, 1.0, size=order + 1) * 10.0 ** (-np.arange(order + 1))
+    c[1] = 5.0
+    poly = np.polynomial.Polynomial(c)
+    grid, coords = line_workload(n, 0, p, xs=poly(i))
+    o = ob.Oracle(grid, *coords, p)
+    h, g = o.metrics(0)
+    sl = slice(3, n - 3)   # away from the reflected ghost coordinates
+    assert np.allclose(h[sl], poly.deriv(1)(i)[sl], rtol=1e-12, atol=1e-11)
+    assert np.allclose(g[sl], poly.deriv(2)(i)[sl], rtol=1e-9, atol=1e-9)
+    # leading error of D on i^(2L+1) at i = 0 (after shifting): 2 sum a_l l^(2L+1)
+    nA, a, b = ob.coeffs(order)
+    assert nA == order // 2
+    lead = {2: 1.0, 4: -4.0, 6: 36.0}[order]          # = (-1)^(L+1) (L!)^2/(2L+1)! * (2L+1)!
+    assert abs(2 * sum(a[l - 1] * l ** (order + 1) for l in range(1, nA + 1)) - lead) < 1e-10
+    assert abs(2 * sum(a[l - 1] * l for l in range(1, nA + 1)) - 1.0) < 1e-15
+    assert abs(sum(b[l - 1] * l * l for l in range(1, nA + 1)) - 1.0) < 1e-15
+
+
+# ------------------------------------------------------------------ P2: Eq. 5-7 index ranges
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_P2_flux_form_equals_split_form(ob, order):
+    """Eq. 6-7 is the locally conservative form of the split convective derivative
+    (refs [32,33]):  d(rho u phi)/dx = 1/4 [ D(rho u phi) + rho D(u phi) + u D(rho phi) + phi D(rho u)
+    + rho u D(phi) + rho phi D(u) + u phi D(rho) ].  Build that with textbook central differences."""
+    p = W.default_params(order=order, viscous_enable=0, Rgas=1 / GAM)
+    wl = W.random_periodic(16, 12, 10, seed=11, params=p)
+    o = make(ob, wl)
+    conv, _ = o.rhs_parts()
+    w = wl.state()
+    rho, u, v, ww, pr = H.cons_to_prim(w, GAM)
+    Hh = (w[4] + pr) / rho
+    vel = [u, v, ww]
+    hs = [wl.x[1] - wl.x[0], wl.y[1] - wl.y[0], wl.z[1] - wl.z[0]]
+    R = np.zeros_like(w)
+    for d, axis in enumerate((2, 1, 0)):
+        D = lambda f: H.ddx(f, axis, hs[d], order)
+        un = vel[d]
+        for m, phi in enumerate([np.ones_like(rho), u, v, ww, Hh]):
+            split = 0.25 * (D(rho * un * phi) + rho * D(un * phi) + un * D(rho * phi) + phi * D(rho * un)
+                            + rho * un * D(phi) + rho * phi * D(un) + un * phi * D(rho))
+            R[m] -= split
+        R[1 + d] -= D(pr)
+    scale = np.abs(R).reshape(5, -1).max(axis=1)[:, None, None, None]
+    assert np.max(np.abs(conv - R) / scale) < 1e-12
+
+
+# ------------------------------------------------------------------ P3: free-stream preservation
+@pytest.mark.parametrize("weno", [0, 1])
+def test_P3_free_stream(ob, weno):
+    p = W.default_params(weno_enable=weno, sensor_threshold=-1.0 if weno else 0.5, Rgas=1 / GAM)
+    wl = W.random_periodic(10, 9, 8, amp=0.0, params=p, stretched_y=True)
+    o = make(ob, wl)
+    r = o.rhs()
+    if weno:
+        d = o.diagnostics()
+        assert list(d.weno_ifaces) == list(d.total_ifaces)      # threshold < 0: every interface is WENO
+        assert np.abs(r).max() < 1e-12
+    else:
+        assert np.abs(r).max() == 0.0                            # bitwise
+
+
+# ------------------------------------------------------------------ P4: discrete conservation
+@pytest.mark.parametrize("weno,stretch", [(0, False), (0, True), (1, False), (1, True)])
+def test_P4_conservation_periodic_inviscid(ob, weno, stretch):
+    p = W.default_params(weno_enable=weno, sensor_threshold=0.02, sensor_eps=0.1, viscous_enable=0, Rgas=1 / GAM)
+    wl = W.random_periodic(14, 12, 10, seed=5, params=p, stretched_y=stretch)
+    o = make(ob, wl)
+    r = o.rhs()
+    d = o.diagnostics()
+    if weno:
+        assert 0 < d.weno_ifaces[0] < d.total_ifaces[0]          # a genuine mix of central and WENO interfaces
+    hx, _ = o.metrics(0)
+    hy, _ = o.metrics(1)
+    hz, _ = o.metrics(2)
+    vol = hz[:, None, None] * hy[None, :, None] * hx[None, None, :]
+    for m in range(5):
+        tot = math.fsum((r[m] * vol).ravel())
+        ref = math.fsum(np.abs(r[m] * vol).ravel())
+        assert abs(tot) < 1e-13 * ref, (m, tot, ref)
+
+
+def test_P4_viscous_sum_is_truncation_level(ob):
+    """Laplacian form (Eq. 9) does not telescope: the momentum sum is small but not round-off."""
+    p = W.default_params(Rgas=1 / GAM, mu_ref=1e-2)
+    wl = W.config1_tgv(16, weno=0)
+    wl.params.update(mu_ref=1e-2)
+    o = make(ob, wl)
+    r = o.rhs()
+    assert abs(math.fsum(r[0].ravel())) < 1e-12 * np.abs(r[0]).sum()          # mass always exact
+    assert abs(math.fsum(r[1].ravel())) < 1e-3 * np.abs(r[1]).sum()
+
+
+# ------------------------------------------------------------------ P5: kinetic-energy preservation
+def test_P5_kinetic_energy_identity(ob):
+    """the central flux conserves kinetic energy discretely.  Semi-discrete identity on
+    periodic data:  sum [u_k R_k - 1/2 |u|^2 R_rho] vol = - sum u_k D_k p vol  (pressure work only)."""
+    p = W.default_params(viscous_enable=0, Rgas=1 / GAM)
+    wl = W.random_periodic(16, 14, 12, seed=9, params=p)
+    o = make(ob, wl)
+    r = o.rhs()
+    w = wl.state()
+    rho, u, v, ww, pr = H.cons_to_prim(w, GAM)
+    hs = [wl.x[1] - wl.x[0], wl.y[1] - wl.y[0], wl.z[1] - wl.z[0]]
+    lhs = u * r[1] + v * r[2] + ww * r[3] - 0.5 * (u * u + v * v + ww * ww) * r[0]
+    rhs = -(u * H.ddx(pr, 2, hs[0]) + v * H.ddx(pr, 1, hs[1]) + ww * H.ddx(pr, 0, hs[2]))
+    scale = math.fsum(np.abs(lhs).ravel())
+    assert abs(math.fsum((lhs - rhs).ravel())) < 1e-13 * scale
+
+
+def test_P5_kinetic_energy_in_time(ob):
+    """Inviscid low-Mach TGV: total kinetic energy changes only through pressure work and the
+    RK3 truncation error, so the KE drift over a fixed time shrinks ~ dt^3 when dt is halved."""
+    drift = []
+    for dt in (0.02, 0.01):
+        wl = W.config1_tgv(12, weno=0)
+        wl.params.update(viscous_enable=0, dt_fixed=dt)
+        o = make(ob, wl)
+        e0 = o.diagnostics().energy
+        k0 = o.diagnostics().kinetic
+        o.step(int(round(0.2 / dt)))
+        d = o.diagnostics()
+        assert abs(d.energy - e0) < 1e-13 * abs(e0)              # total energy conserved to round-off
+        drift.append(d.kinetic - k0)
+    assert abs(drift[0] - drift[1]) < 2e-3 * abs(k0)             # KE insensitive to dt: no numerical dissipation
+
+
+# ------------------------------------------------------------------ P6: RK3 (reading G5)
+def test_P6_rk3_order_conditions_rational():
+    al = [Fraction(0), Fraction(-17, 60), Fraction(-5, 12)]
+    be = [Fraction(8, 15), Fraction(5, 12), Fraction(3, 4)]
+    # Butcher form of w^(l+1) = w^(l) + dt (alpha_l R^(l-1) + beta_l R^(l))
+    a21 = be[0]
+    a31, a32 = be[0] + al[1], be[1]
+    b1, b2, b3 = a31, a32 + al[2], be[2]
+    c2, c3 = a21, a31 + a32
+    assert (b1, b2, b3) == (Fraction(1, 4), 0, Fraction(3, 4)) and (c2, c3) == (Fraction(8, 15), Fraction(2, 3))
+    assert b1 + b2 + b3 == 1 and b2 * c2 + b3 * c3 == Fraction(1, 2)
+    assert b2 * c2 ** 2 + b3 * c3 ** 2 == Fraction(1, 3) and b3 * a32 * c2 == Fraction(1, 6)
+    # the printed alpha_1 = +17/60 is not even first-order consistent
+    assert sum(be) + Fraction(17, 60) + al[2] != 1
+
+
+def test_P6_rk3_matches_butcher_tableau(ob):
+    """One oracle step == textbook Wray RK3 (c = 0, 8/15, 2/3; b = 1/4, 0, 3/4) driven by oracle.rhs()."""
+    dt = 0.01
+    wl = W.config1_tgv(8, weno=0)
+    wl.params.update(dt_fixed=dt)
+    o = make(ob, wl)
+    w0 = wl.state()
+    k1 = o.rhs()
+    o.set_state(w0 + dt * (8 / 15) * k1)
+    k2 = o.rhs()
+    o.set_state(w0 + dt * (1 / 4 * k1 + 5 / 12 * k2))
+    k3 = o.rhs()
+    ref = w0 + dt * (1 / 4 * k1 + 3 / 4 * k3)
+    o.set_state(w0)
+    o.step(1)
+    got = o.get_state()
+    assert np.max(np.abs(got - ref)) < 1e-13 * np.abs(ref).max()
+    assert abs(o.diagnostics().time - dt) < 1e-16
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_P6_rk3_third_order_entropy_wave(ob, d):
+    """rho = 1 + 0.2 sin(x - t), u = 1, p = 1 is an exact Euler solution.  Temporal error vs a
+    fine-dt run on the same grid must fall by ~8 when dt is halved."""
+    n = 32
+    L = 2 * np.pi
+    p = W.default_params(viscous_enable=0, Rgas=1 / GAM)
+    grid, coords = line_workload(n, d, p, L=L)
+    xs = coords[d]
+    vel = [0.0, 0.0, 0.0]
+    vel[d] = 1.0
+    shape = (grid["nz"], grid["ny"], grid["nx"])
+    rho = (1 + 0.2 * np.sin(xs)).reshape(shape)
+    w0 = W.prim_to_cons(rho, vel[0] + 0 * rho, vel[1] + 0 * rho, vel[2] + 0 * rho, np.ones(shape), GAM)
+
+    def run(dt, T=0.4):
+        pp = dict(p, dt_fixed=dt)
+        o = ob.Oracle(grid, *coords, pp)
+        o.set_state(w0)
+        o.step(int(round(T / dt)))
+        return o.get_state()
+
+    ref = run(0.00125)
+    e1 = np.abs(run(0.04) - ref).max()
+    e2 = np.abs(run(0.02) - ref).max()
+    assert 6.5 < e1 / e2 < 9.5, e1 / e2
+    exact = 1 + 0.2 * np.sin(xs - 0.4)
+    assert np.abs(ref[0].ravel() - exact).max() < 5e-6          # and the scheme converges to the exact solution
+
+
+# ------------------------------------------------------------------ P7: eigenvectors
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_P7_eigenvectors(ob, d):
+    rng = np.random.default_rng(d)
+    ub = rng.uniform(-1, 1, 3)
+    c = 1.3
+    Hb = c * c / (GAM - 1) + 0.5 * ub @ ub
+    Lm, Rm, lam = ob.eigen(d, GAM, ub, Hb)
+    assert np.allclose(Lm @ Rm, np.eye(5), atol=1e-14)
+    rho = 0.9
+    pres = rho * c * c / GAM
+    wv = np.array([rho, rho * ub[0], rho * ub[1], rho * ub[2], pres / (GAM - 1) + 0.5 * rho * ub @ ub])
+    J = np.zeros((5, 5))
+    for m in range(5):
+        wc = wv.astype(complex)
+        wc[m] += 1e-30j
+        J[:, m] = H.euler_flux(wc, d, GAM).imag / 1e-30
+    assert np.allclose(Rm @ np.diag(lam) @ Lm, J, atol=1e-12)
+    assert np.allclose(lam, [ub[d] - c, ub[d], ub[d], ub[d], ub[d] + c])
+
+
+# ------------------------------------------------------------------ P8: WENO5
+def test_P8_weno5_limits(ob):
+    rng = np.random.default_rng(0)
+    for _ in range(5):
+        s, t = rng.uniform(-2, 2, 2)
+        v = [s * i + t for i in range(5)]
+        assert abs(ob.weno5(*v) - (2 * v[0] - 13 * v[1] + 47 * v[2] + 27 * v[3] - 3 * v[4]) / 60) < 1e-14
+    # smooth data: cell averages of sin -> interface value, fifth order
+    errs = []
+    for h in (0.2, 0.1):
+        x0 = 0.3
+        avg = lambda a, b: (math.cos(a) - math.cos(b)) / (b - a)
+        v = [avg(x0 + (i - 2.5) * h, x0 + (i - 1.5) * h) for i in range(5)]
+        errs.append(abs(ob.weno5(*v) - math.sin(x0 + 0.5 * h)))
+    assert 20 < errs[0] / errs[1] < 45
+    # discontinuity inside the right part of the stencil: essentially the left-biased candidate
+    val = ob.weno5(1.0, 1.0, 1.0, 0.0, 0.0)
+    assert abs(val - 1.0) < 1e-6
+
+
+# ------------------------------------------------------------------ P9: Sod tube, hybrid recipe end to end
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_P9_sod_tube(ob, d):
+    errs = []
+    for n in (100, 200):
+        xs = (np.arange(n) + 0.5) / n
+        bc = [W.BC_PERIODIC] * 6
+        bc[2 * d] = bc[2 * d + 1] = W.BC_EXTRAP
+        p = W.default_params(viscous_enable=0, weno_enable=1, sensor_threshold=0.5, sensor_eps=1e-6,
+                             Rgas=1.0, cfl=0.5, bc=bc)
+        grid, coords = line_workload(n, d, p, xs=xs)
+        shape = (grid["nz"], grid["ny"], grid["nx"])
+        left = (xs < 0.5).reshape(shape)
+        rho = np.where(left, 1.0, 0.125)
+        pres = np.where(left, 1.0, 0.1)
+        zero = np.zeros(shape)
+        o = ob.Oracle(grid, *coords, p)
+        o.set_state(W.prim_to_cons(rho, zero, zero, zero, pres, GAM))
+        while True:
+            o.step(1)
+            dg = o.diagnostics()
+            if dg.time >= 0.2:
+                break
+        w = o.get_state()
+        assert dg.min_rho > 0.12 and dg.min_p > 0.09
+        assert dg.weno_ifaces[d] > 0 and dg.weno_ifaces[d] < dg.total_ifaces[d] // 2
+        r_ex, u_ex, p_ex, pstar, ustar = H.exact_riemann(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, GAM, (xs - 0.5) / dg.time)
+        assert abs(pstar - 0.303130) < 1e-5 and abs(ustar - 0.927453) < 1e-5
+        errs.append(np.abs(w[0].ravel() - r_ex).mean())
+        mom = w[1 + d].ravel() / w[0].ravel()
+        assert np.abs(mom - u_ex).mean() < 0.02
+        for t in range(3):
+            if t != d:
+                assert np.abs(w[1 + t]).max() < 1e-13
+    assert errs[0] < 8e-3 and errs[1] < 4e-3 and errs[1] < 0.65 * errs[0], errs
+
+
+# ------------------------------------------------------------------ P10: shock generator
+def test_P10_oblique_shock(ob):
+    M = 2.28
+    p = W.default_params(Rgas=1 / GAM, fs=[1.0, M, 0.0, 0.0, 1.0], shock_angle_deg=8.0)
+    post, beta = ob.shock_state(p)
+    rho2, u2, v2, w2, T2 = post
+    assert abs(math.degrees(beta) - 32.68526) < 1e-4
+    assert abs(rho2 - 1.395939) < 1e-6 and abs(T2 - 1.147604) < 1e-6
+    assert abs(u2 - 2.091408) < 1e-6 and abs(v2 + 0.293928) < 1e-6 and w2 == 0.0
+    assert abs(math.degrees(math.atan2(-v2, u2)) - 8.0) < 1e-9            # deflection
+    # Rankine-Hugoniot across the shock plane with normal (sin b, cos b)
+    nx_, ny_ = math.sin(beta), math.cos(beta)
+    p1, p2 = 1 / GAM, rho2 * T2 / GAM
+    un1, un2 = M * nx_, u2 * nx_ + v2 * ny_
+    assert abs(1.0 * un1 - rho2 * un2) < 1e-12
+    assert abs(un1 ** 2 + p1 - rho2 * un2 ** 2 - p2) < 1e-12
+    h1 = GAM / (GAM - 1) * p1 + 0.5 * M * M
+    h2 = GAM / (GAM - 1) * p2 / rho2 + 0.5 * (u2 * u2 + v2 * v2)
+    assert abs(h1 - h2) < 1e-12
+    assert abs((M * ny_) - (u2 * ny_ - v2 * nx_)) < 1e-12               # tangential velocity kept
+    assert abs(p2 / p1 - 1.601985) < 1e-6
+
+
+# ------------------------------------------------------------------ P11/P12: staggered wall and forcing
+def test_P11_P12_channel_mass_and_bulk_momentum(ob):
+    wl = W.config3_channel(16, 16, 8, steps=10)
+    o = make(ob, wl)
+    d0 = o.diagnostics()
+    r = o.rhs()
+    hx, _ = o.metrics(0)
+    hy, _ = o.metrics(1)
+    hz, _ = o.metrics(2)
+    vol = hz[:, None, None] * hy[None, :, None] * hx[None, None, :]
+    assert abs(math.fsum((r[0] * vol).ravel())) < 1e-13 * np.abs(r[0] * vol).sum()   # wall mass flux exactly 0
+    assert abs(math.fsum((r[1] * vol).ravel())) < 1e-13 * np.abs(r[1] * vol).sum()   # forcing cancels the drag
+    assert o.diagnostics().forcing > 0.0                                            # Poiseuille start needs f > 0
+    o.step(10)
+    d1 = o.diagnostics()
+    assert abs(d1.mass - d0.mass) < 1e-13 * d0.mass
+    assert abs(d1.mom[0] - d0.mom[0]) < 1e-13 * abs(d0.mom[0])
+    assert abs(d0.volume - 6 * np.pi * 2 * 2 * np.pi) < 1e-3 * d0.volume
+    # uniform flow at rest between walls at the gas temperature: nothing happens, f = 0
+    wl2 = W.config3_channel(8, 8, 4)
+    w = wl2.state()
+    w[1:4] = 0.0
+    w[4] = (1 / GAM) / (GAM - 1)
+    o2 = ob.Oracle(wl2.grid, wl2.x, wl2.y, wl2.z, wl2.params)
+    o2.set_state(w)
+    assert np.abs(o2.rhs()).max() < 1e-13
+    assert abs(o2.diagnostics().forcing) < 1e-15
+
+
+# ------------------------------------------------------------------ P13: time step
+def test_P13_dt_closed_form(ob):
+    p = W.default_params(Rgas=1 / GAM, cfl=0.5)
+    wl = W.random_periodic(8, 6, 4, amp=0.0, params=p)      # u = (0.5, 0, -0.3), c = 1
+    o = make(ob, wl)
+    o.step(1)
+    hs = [2 * np.pi / 8, 2 * np.pi / 6, 2 * np.pi / 4]
+    expect = 0.5 / max(1.5 / hs[0], 1.0 / hs[1], 1.3 / hs[2])
+    assert abs(o.diagnostics().dt - expect) < 1e-14
+
+
+# ------------------------------------------------------------------ P14: non-reflecting outflow
+def test_P14_outflow(ob):
+    bc = [W.BC_INFLOW, W.BC_OUTFLOW] + [W.BC_PERIODIC] * 4
+    p = W.default_params(Rgas=1 / GAM, viscous_enable=0, bc=bc)
+    n = 64
+    xs = np.arange(n) / n
+    grid, coords = line_workload(n, 0, p, xs=xs)
+    shape = (1, 1, n)
+    one = np.ones(shape)
+    o = ob.Oracle(grid, *coords, p)
+    o.set_state(W.prim_to_cons(one, 2.0 * one, 0 * one, 0 * one, one / GAM, GAM))   # uniform M = 2
+    assert np.abs(o.rhs()).max() == 0.0
+    # subsonic acoustic pulse leaving through the outflow: reflected amplitude << incident
+    amp = 1e-3
+    pulse = amp * np.exp(-((xs - 0.6) / 0.05) ** 2).reshape(shape)
+    rho = one + pulse
+    pres = one / GAM + pulse                  # right-running simple wave (c = 1, rho c = 1): p' = rho' = u'
+    u = 0.3 * one + pulse
+    o.set_state(W.prim_to_cons(rho, u, 0 * one, 0 * one, pres, GAM))
+    while o.diagnostics().time < 0.55:
+        o.step(1)
+    w = o.get_state()
+    resid = np.abs(w[0].ravel()[8:] - 1.0).max()   # skip the frozen-inflow neighbourhood
+    assert resid < 0.05 * amp, resid
+
+
+# ------------------------------------------------------------------ P15: metrics on stretched grids
+def test_P15_metrics_order(ob):
+    errs = []
+    for ny in (32, 64):
+        wl = W.config3_channel(4, ny, 4)
+        o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+        h, g = o.metrics(1)
+        b = 1.7
+        eta = -1 + (2 * np.arange(1, ny + 1) - 1) / ny
+        deta = 2.0 / ny
+        dy = b / np.cosh(b * eta) ** 2 / np.tanh(b) * deta               # dy/dj analytic
+        errs.append(np.abs(h / dy - 1)[4:-4].max())
+    assert errs[0] / errs[1] > 40, errs                                    # sixth order (64 ideal)
+    wl = W.random_periodic(8, 8, 8)
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    h, g = o.metrics(0)
+    assert np.allclose(h, 2 * np.pi / 8, rtol=1e-14) and np.abs(g).max() < 1e-14
+
+
+# ------------------------------------------------------------------ P16 + design order: manufactured fields
+@pytest.fixture(scope="module")
+def manufactured():
+    import sympy as sp
+    x, y, z = sp.symbols("x y z")
+    R, mu0, expo, Pr = sp.Rational(5, 7), sp.Rational(1, 50), sp.Rational(19, 25), sp.Rational(18, 25)
+    gam = sp.Rational(7, 5)
+    rho = 1 + sp.Rational(1, 10) * sp.sin(x + y) * sp.cos(z)
+    vel = [sp.Rational(1, 2) + sp.Rational(1, 5) * sp.sin(x) * sp.cos(2 * y) * sp.cos(z),
+           sp.Rational(1, 5) * sp.cos(x + z) * sp.sin(y),
+           -sp.Rational(3, 10) + sp.Rational(1, 5) * sp.sin(2 * x - y) * sp.sin(z)]
+    T = 1 + sp.Rational(1, 10) * sp.cos(x - y + z)
+    p = rho * R * T
+    mu = mu0 * T ** expo
+    X = [x, y, z]
+    th = sum(sp.diff(vel[i], X[i]) for i in range(3))
+    sig = [[mu * (sp.diff(vel[i], X[j]) + sp.diff(vel[j], X[i]) - (sp.Rational(2, 3) * th if i == j else 0))
+            for j in range(3)] for i in range(3)]
+    cp = gam * R / (gam - 1)
+    q = [-cp * mu / Pr * sp.diff(T, X[j]) for j in range(3)]
+    Vm = [sum(sp.diff(sig[i][j], X[j]) for j in range(3)) for i in range(3)]
+    VE = sum(sp.diff(sum(sig[i][j] * vel[i] for i in range(3)) - q[j], X[j]) for j in range(3))
+    E = R / (gam - 1) * T + sum(c * c for c in vel) / 2
+    Hh = E + p / rho
+    conv = [-sum(sp.diff(rho * vel[j], X[j]) for j in range(3))]
+    conv += [-sum(sp.diff(rho * vel[i] * vel[j], X[j]) for j in range(3)) - sp.diff(p, X[i]) for i in range(3)]
+    conv += [-sum(sp.diff(rho * vel[j] * Hh, X[j]) for j in range(3))]
+    f = sp.lambdify((x, y, z), [rho, *vel, p] + Vm + [VE] + conv, "numpy")
+    return f
+
+
+@pytest.mark.parametrize("stretch", [False, True])
+def test_P16_viscous_and_convective_design_order(ob, manufactured, stretch):
+    errs_v, errs_c = [], []
+    for n in (12, 24):
+        L = 2 * np.pi
+        xs = L * np.arange(n) / n
+        ys = xs + (0.25 * np.sin(xs) if stretch else 0.0)
+        p = W.default_params(Rgas=5 / 7, mu_ref=1 / 50, T_ref=1.0, visc_exp=0.76, Pr=0.72)
+        grid = dict(nx=n, ny=n, nz=n, len=[L, L, L])
+        Z, Y, X = np.meshgrid(xs, ys, xs, indexing="ij")
+        vals = [np.broadcast_to(np.asarray(a, dtype=float), X.shape) for a in manufactured(X, Y, Z)]
+        rho, u, v, w, pr = vals[:5]
+        Vex = vals[5:9]
+        Cex = vals[9:14]
+        o = ob.Oracle(grid, xs, ys, xs, p)
+        o.set_state(W.prim_to_cons(rho, u, v, w, pr, GAM))
+        conv, visc = o.rhs_parts()
+        assert np.abs(visc[0]).max() == 0.0
+        errs_v.append(max(np.abs(visc[1 + m] - Vex[m]).max() / np.abs(Vex[m]).max() for m in range(4)))
+        errs_c.append(max(np.abs(conv[m] - Cex[m]).max() / np.abs(Cex[m]).max() for m in range(5)))
+    assert errs_v[1] < 5e-4 and errs_v[0] / errs_v[1] > 30, errs_v      # sixth order: 64 ideal
+    assert errs_c[1] < 5e-4 and errs_c[0] / errs_c[1] > 30, errs_c
+
+
+def test_P16_one_dimensional_reduction_of_eq9(ob):
+    """1-D field u(x), constant T: the x-momentum viscous term must be (4/3) [mu u_xx + mu_x u_x] with
+    mu_x = 0, i.e. 4/3 mu D2 u / dx^2 with the b_l of the table (Eq. 9)."""
+    n = 16
+    L = 2 * np.pi
+    xs = L * np.arange(n) / n
+    p = W.default_params(Rgas=1 / GAM, mu_ref=0.01)
+    grid, coords = line_workload(n, 0, p, L=L)
+    u = (0.1 * np.sin(xs)).reshape(1, 1, n)
+    one = np.ones_like(u)
+    o = ob.Oracle(grid, *coords, p)
+    o.set_state(W.prim_to_cons(one, u, 0 * one, 0 * one, one / GAM, GAM))
+    _, visc = o.rhs_parts()
+    b = [3 / 2, -3 / 20, 1 / 90]
+    uu = u.ravel()
+    d2 = sum(b[l - 1] * (np.roll(uu, -l) - 2 * uu + np.roll(uu, l)) for l in (1, 2, 3)) / (L / n) ** 2
+    assert np.allclose(visc[1].ravel(), 4 / 3 * 0.01 * d2, rtol=1e-11, atol=1e-15)
+
+
+# ------------------------------------------------------------------ sensor sanity (Eq. 8)
+def test_sensor_range_and_limits(ob):
+    """theta in [0,1]; ~0 for solenoidal vortical flow (TGV), ~1 in a pure compression."""
+    wl = W.config1_tgv(16)
+    o = make(ob, wl)
+    th, fl = o.sensor()
+    assert th.min() >= 0.0 and th.max() <= 1.0 and th.max() < 0.1 and fl.sum() == 0
+    n = 32
+    p = W.default_params(Rgas=1 / GAM, weno_enable=1, sensor_eps=1e-8)
+    grid, coords = line_workload(n, 0, p, L=2 * np.pi)
+    u = (-0.5 * np.sin(coords[0])).reshape(1, 1, n)      # compression at x = 0, expansion at x = pi
+    one = np.ones_like(u)
+    o = ob.Oracle(grid, *coords, p)
+    o.set_state(W.prim_to_cons(one, u, 0 * one, 0 * one, one / GAM, GAM))
+    th, fl = o.sensor()
+    assert th.ravel()[0] > 0.999 and th.ravel()[n // 2] == 0.0
+    assert fl[0].ravel()[0] == 1 and fl[0].ravel()[n // 2] == 0
+    # interface flag = any of the six stencil nodes above threshold
+    node = th.ravel() > 0.5
+    exp = np.array([any(node[(i + s) % n] for s in range(-2, 4)) for i in range(n)])
+    assert np.array_equal(fl[0].ravel().astype(bool), exp)
