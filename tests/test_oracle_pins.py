@@ -463,7 +463,7 @@ def manufactured():
 @pytest.mark.parametrize("stretch", [False, True])
 def test_P16_viscous_and_convective_design_order(ob, manufactured, stretch):
     errs_v, errs_c = [], []
-    for n in (12, 24):
+    for n in (16, 32):
         L = 2 * np.pi
         xs = L * np.arange(n) / n
         ys = xs + (0.25 * np.sin(xs) if stretch else 0.0)
@@ -480,8 +480,8 @@ def test_P16_viscous_and_convective_design_order(ob, manufactured, stretch):
         assert np.abs(visc[0]).max() == 0.0
         errs_v.append(max(np.abs(visc[1 + m] - Vex[m]).max() / np.abs(Vex[m]).max() for m in range(4)))
         errs_c.append(max(np.abs(conv[m] - Cex[m]).max() / np.abs(Cex[m]).max() for m in range(5)))
-    assert errs_v[1] < 5e-4 and errs_v[0] / errs_v[1] > 30, errs_v      # sixth order: 64 ideal
-    assert errs_c[1] < 5e-4 and errs_c[0] / errs_c[1] > 30, errs_c
+    assert errs_v[1] < 1e-4 and errs_v[0] / errs_v[1] > 40, errs_v      # sixth order: 64 ideal
+    assert errs_c[1] < 1e-4 and errs_c[0] / errs_c[1] > 40, errs_c
 
 
 def test_P16_one_dimensional_reduction_of_eq9(ob):
