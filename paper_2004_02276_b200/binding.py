@@ -1,0 +1,220 @@
+"""Thin ctypes binding of the C-ABI library declared in include/streams.h.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of
+libstreams_b200.so.  PyTorch is used for device memory and the CUDA stream, nothing else.
+There is no CPU fallback: if the library is missing or no GPU is present, calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libstreams_b200.so")
+
+STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, STREAMS_ESTATE = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
+           "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
+           "streams_diagnostics", "streams_launch_count", "streams_last_error", "streams_destroy"]
+
+
+class StreamsGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("pad_", C.c_int), ("len", C.c_double * 3)]
+
+
+class StreamsParams(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("Pr", C.c_double), ("Rgas", C.c_double), ("mu_ref", C.c_double),
+                ("T_ref", C.c_double), ("visc_exp", C.c_double), ("suth_S", C.c_double),
+                ("sensor_threshold", C.c_double), ("sensor_eps", C.c_double),
+                ("T_wall", C.c_double * 2), ("y_wall", C.c_double * 2), ("fs", C.c_double * 5),
+                ("shock_angle_deg", C.c_double), ("x_shock", C.c_double), ("cfl", C.c_double),
+                ("dt_fixed", C.c_double),
+                ("visc_model", C.c_int), ("order", C.c_int), ("weno_enable", C.c_int), ("forcing", C.c_int),
+                ("viscous_enable", C.c_int), ("bc", C.c_int * 6), ("pad_", C.c_int)]
+
+
+class StreamsDiag(C.Structure):
+    _fields_ = [("step", C.c_longlong), ("time", C.c_double), ("dt", C.c_double), ("forcing", C.c_double),
+                ("mass", C.c_double), ("mom", C.c_double * 3), ("energy", C.c_double), ("kinetic", C.c_double),
+                ("volume", C.c_double), ("bulk_rhou", C.c_double),
+                ("min_rho", C.c_double), ("min_p", C.c_double), ("max_mach", C.c_double), ("max_theta", C.c_double),
+                ("max_speed", C.c_double * 3),
+                ("weno_ifaces", C.c_longlong * 3), ("total_ifaces", C.c_longlong * 3),
+                ("nonfinite", C.c_int), ("pad_", C.c_int)]
+
+
+class StreamsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"streams error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+_DBL = C.POINTER(C.c_double)
+
+
+def lib():
+    """Load libstreams_b200.so (built by paper_2004_02276_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2004_02276_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.streams_workspace_bytes.argtypes = [C.POINTER(StreamsGrid), C.POINTER(StreamsParams)]
+        L.streams_workspace_bytes.restype = C.c_size_t
+        L.streams_create.argtypes = [C.POINTER(StreamsGrid), _DBL, _DBL, _DBL, C.POINTER(StreamsParams),
+                                     C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+        for name in ("streams_set_state", "streams_set_state_host", "streams_get_state", "streams_get_state_host",
+                     "streams_rhs"):
+            getattr(L, name).argtypes = [C.c_void_p, C.c_void_p]
+        L.streams_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.streams_step.argtypes = [C.c_void_p, C.c_int]
+        L.streams_diagnostics.argtypes = [C.c_void_p, C.POINTER(StreamsDiag)]
+        L.streams_launch_count.argtypes = [C.c_void_p]
+        L.streams_launch_count.restype = C.c_longlong
+        L.streams_last_error.argtypes = [C.c_void_p]
+        L.streams_last_error.restype = C.c_char_p
+        L.streams_destroy.argtypes = [C.c_void_p]
+        L.streams_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def make_params(params: dict) -> StreamsParams:
+    p = StreamsParams()
+    for name, _t in StreamsParams._fields_:
+        if name == "pad_":
+            continue
+        v = params[name]
+        if isinstance(v, (list, tuple, np.ndarray)):
+            arr = getattr(p, name)
+            for i, x in enumerate(v):
+                arr[i] = x
+        else:
+            setattr(p, name, v)
+    return p
+
+
+def make_grid(grid: dict) -> StreamsGrid:
+    g = StreamsGrid()
+    g.nx, g.ny, g.nz = int(grid["nx"]), int(grid["ny"]), int(grid["nz"])
+    for i in range(3):
+        g.len[i] = grid["len"][i]
+    return g
+
+
+def workspace_bytes(grid: dict, params: dict) -> int:
+    g, p = make_grid(grid), make_params(params)
+    return lib().streams_workspace_bytes(C.byref(g), C.byref(p))
+
+
+class Streams:
+    """One context of the CUDA library.  Device buffers are torch tensors owned by this object."""
+
+    def __init__(self, grid: dict, x, y, z, params: dict, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2004_02276_b200 needs a CUDA device (no CPU fallback)")
+        self._torch = torch
+        self.device = torch.device(device)
+        self.n = (int(grid["nx"]), int(grid["ny"]), int(grid["nz"]))
+        self.shape = (5, self.n[2], self.n[1], self.n[0])
+        self._g, self._p = make_grid(grid), make_params(params)
+        self._h = None
+        nbytes = lib().streams_workspace_bytes(C.byref(self._g), C.byref(self._p))
+        if nbytes == 0:
+            raise StreamsError(STREAMS_EINVAL, "invalid grid/params")
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            xs = [np.ascontiguousarray(a, dtype=np.float64) for a in (x, y, z)]
+            h = C.c_void_p()
+            rc = lib().streams_create(C.byref(self._g), xs[0].ctypes.data_as(_DBL), xs[1].ctypes.data_as(_DBL),
+                                      xs[2].ctypes.data_as(_DBL), C.byref(self._p), C.c_void_p(self._ws.data_ptr()),
+                                      nbytes, C.c_void_p(self._stream.cuda_stream), C.byref(h))
+        if rc != 0:
+            raise StreamsError(rc, lib().streams_last_error(None).decode())
+        self._h = h
+        self.workspace_bytes = nbytes
+
+    def close(self):
+        if self._h:
+            lib().streams_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc, allow=()):
+        if rc != 0 and rc not in allow:
+            raise StreamsError(rc, lib().streams_last_error(self._h).decode())
+        return rc
+
+    def _dev(self, t, shape=None, dtype=None):
+        torch = self._torch
+        dtype = dtype or torch.float64
+        assert t.is_cuda and t.dtype == dtype and t.is_contiguous(), "need a contiguous CUDA tensor"
+        if shape is not None:
+            assert tuple(t.shape) == tuple(shape), (tuple(t.shape), shape)
+        return C.c_void_p(t.data_ptr())
+
+    # --- state --------------------------------------------------------------------------------
+    def set_state(self, w):
+        """w: torch CUDA tensor [5][nz][ny][nx] (device path) or NumPy array (host path)."""
+        if isinstance(w, np.ndarray):
+            w = np.ascontiguousarray(w, dtype=np.float64)
+            assert w.shape == self.shape
+            self._chk(lib().streams_set_state_host(self._h, C.c_void_p(w.ctypes.data)))
+        else:
+            self._chk(lib().streams_set_state(self._h, self._dev(w, self.shape)))
+
+    def set_state_host_ptr(self, ptr):
+        self._chk(lib().streams_set_state_host(self._h, C.c_void_p(ptr)))
+
+    def get_state_host_ptr(self, ptr):
+        self._chk(lib().streams_get_state_host(self._h, C.c_void_p(ptr)))
+
+    def get_state(self, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().streams_get_state(self._h, self._dev(out, self.shape)))
+        return out
+
+    def get_state_host(self):
+        out = np.empty(self.shape)
+        self._chk(lib().streams_get_state_host(self._h, C.c_void_p(out.ctypes.data)))
+        return out
+
+    # --- hot path -------------------------------------------------------------------------------
+    def rhs(self, out=None):
+        torch = self._torch
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().streams_rhs(self._h, self._dev(out, self.shape)))
+        return out
+
+    def sensor(self):
+        torch = self._torch
+        th = torch.empty(self.shape[1:], dtype=torch.float64, device=self.device)
+        fl = torch.empty((3,) + self.shape[1:], dtype=torch.uint8, device=self.device)
+        self._chk(lib().streams_sensor(self._h, C.c_void_p(th.data_ptr()), C.c_void_p(fl.data_ptr())))
+        return th, fl
+
+    def step(self, n=1):
+        self._chk(lib().streams_step(self._h, int(n)))
+
+    def diagnostics(self, check=True):
+        d = StreamsDiag()
+        rc = lib().streams_diagnostics(self._h, C.byref(d))
+        self._chk(rc, allow=() if check else (STREAMS_ENONFINITE,))
+        return d
+
+    def launch_count(self):
+        return lib().streams_launch_count(self._h)

@@ -1,0 +1,260 @@
+// k_weno.cuh -- shock sensor (a3) and the WENO5 correction on flagged interfaces (a5).
+//
+// The hybrid switch is hard (A6): interface i+1/2 takes the characteristic-wise
+// Lax-Friedrichs WENO5 flux when any of its six stencil nodes has theta > theta_th, the
+// central flux otherwise.  The fused kernel evaluates the central flux
+// everywhere; here the few flagged interfaces add  dF = F_weno - F_central  to their two
+// nodes.  Work is compacted: k_weno_list appends every node with at least one flagged
+// interface, k_weno_apply runs one thread per listed node (no divergence on clean warps, no
+// floating-point atomics: each node sums its own corrections in a fixed order).
+#pragma once
+#include "dev_common.cuh"
+#include "k_aux.cuh"
+
+namespace streams {
+
+// ---- S4: theta of Eq. 8 per node -> byte flag theta > theta_th ----
+__global__ void __launch_bounds__(RT) k_sensor(const DevP P, const double* __restrict__ w, unsigned char* __restrict__ nflag,
+                                               double* __restrict__ theta_out, DevScal* sc) {
+  __shared__ double sh[RT / 32];
+  double tmax = 0.0;
+  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+#pragma unroll
+      for (int l = 1; l <= 3; ++l) {
+        double up, vp, wp, um, vm, wm;
+        fetch_vel(P, w, i + (d == 0 ? l : 0), j + (d == 1 ? l : 0), k + (d == 2 ? l : 0), up, vp, wp);
+        fetch_vel(P, w, i - (d == 0 ? l : 0), j - (d == 1 ? l : 0), k - (d == 2 ? l : 0), um, vm, wm);
+        const double a = P.c.a[l - 1];
+        G[0][d] += a * (up - um); G[1][d] += a * (vp - vm); G[2][d] += a * (wp - wm);
+      }
+    }
+    const double ih[3] = {P.ih[0][i], P.ih[1][j], P.ih[2][k]};
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int d = 0; d < 3; ++d) G[a][d] *= ih[d];
+    const double div = G[0][0] + G[1][1] + G[2][2];
+    const double ox = G[2][1] - G[1][2], oy = G[0][2] - G[2][0], oz = G[1][0] - G[0][1];
+    const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
+    nflag[o] = th > P.th_thr ? 1 : 0;
+    if (theta_out) theta_out[o] = th;
+    tmax = fmax(tmax, th);
+  }
+  const double t = block_max<RT>(tmax, sh, threadIdx.x);
+  if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned long long*>(&sc->max_theta), (unsigned long long)__double_as_longlong(t));
+}
+
+// node flag at a (possibly ghost) index along direction d: periodic wrap, else nearest interior node (A17)
+__device__ __forceinline__ int nflag_at(const DevP& P, const unsigned char* __restrict__ nflag, int d, int i, int j, int k, int g) {
+  const int n = d == 0 ? P.nx : (d == 1 ? P.ny : P.nz);
+  const int gg = P.bc[2 * d] == BC_PERIODIC ? wrap(g, n) : min(max(g, 0), n - 1);
+  const int ii = d == 0 ? gg : i, jj = d == 1 ? gg : j, kk = d == 2 ? gg : k;
+  return nflag[((size_t)kk * P.ny + jj) * P.nx + ii];
+}
+// interface f+1/2 along d (between nodes f and f+1) flagged?  (A6; the staggered wall plane never is)
+__device__ __forceinline__ int iface_flag(const DevP& P, const unsigned char* __restrict__ nflag, int d, int i, int j, int k, int f) {
+  const int n = d == 0 ? P.nx : (d == 1 ? P.ny : P.nz);
+  if ((f == -1 && P.bc[2 * d] == BC_WALL_STAG) || (f == n - 1 && P.bc[2 * d + 1] == BC_WALL_STAG)) return 0;
+  int any = 0;
+#pragma unroll
+  for (int g = -2; g <= 3; ++g) any |= nflag_at(P, nflag, d, i, j, k, f + g);
+  return any;
+}
+
+// list of nodes with a flagged interface; entry = node index, mask bit (2d+side), side 0 = below, 1 = above
+__global__ void __launch_bounds__(RT) k_weno_list(const DevP P, const unsigned char* __restrict__ nflag,
+                                                  unsigned int* __restrict__ list, unsigned char* __restrict__ lmask,
+                                                  unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
+  unsigned long long cnt[3] = {0, 0, 0};
+  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    const int id[3] = {i, j, k};
+    int mask = 0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const int lo = iface_flag(P, nflag, d, i, j, k, id[d] - 1);
+      const int hi = iface_flag(P, nflag, d, i, j, k, id[d]);
+      mask |= (lo << (2 * d)) | (hi << (2 * d + 1));
+      cnt[d] += hi;
+      if (id[d] == 0 && P.bc[2 * d] != BC_PERIODIC) cnt[d] += lo;
+      if (iflags_out) iflags_out[d * P.N + o] = (unsigned char)hi;
+    }
+    if (mask && list) {
+      const unsigned int pos = atomicAdd(&sc->list_count, 1u);
+      list[pos] = (unsigned int)o;
+      lmask[pos] = (unsigned char)mask;
+    }
+  }
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    for (int s = 16; s > 0; s >>= 1) cnt[d] += __shfl_down_sync(0xffffffffu, cnt[d], s);
+    if ((threadIdx.x & 31) == 0 && cnt[d]) atomicAdd(&sc->weno_if[d], cnt[d]);
+  }
+}
+
+__device__ __forceinline__ double weno5(double a, double b, double c, double d, double e) {
+  const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) * (1.0 / 6.0);
+  const double q1 = (-b + 5.0 * c + 2.0 * d) * (1.0 / 6.0);
+  const double q2 = (2.0 * c + 5.0 * d - e) * (1.0 / 6.0);
+  const double t0 = a - 2.0 * b + c, u0 = a - 4.0 * b + 3.0 * c;
+  const double t1 = b - 2.0 * c + d, u1 = b - d;
+  const double t2 = c - 2.0 * d + e, u2 = 3.0 * c - 4.0 * d + e;
+  const double b0 = (13.0 / 12.0) * t0 * t0 + 0.25 * u0 * u0;
+  const double b1 = (13.0 / 12.0) * t1 * t1 + 0.25 * u1 * u1;
+  const double b2 = (13.0 / 12.0) * t2 * t2 + 0.25 * u2 * u2;
+  const double eps = 1e-6;
+  const double a0 = 0.1 / ((eps + b0) * (eps + b0));
+  const double a1 = 0.6 / ((eps + b1) * (eps + b1));
+  const double a2 = 0.3 / ((eps + b2) * (eps + b2));
+  return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
+}
+
+// dF = F_weno - F_central at the interface between node (i,j,k) and its upper neighbour along D (S5, S6)
+template <int D>
+__device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, int j, int k, double dF[5]) {
+  double rho[6], vel[6][3], Hh[6], pp[6], cs[6];
+#pragma unroll
+  for (int n = 0; n < 6; ++n) {
+    const int off = n - 2;
+    Prim q;
+    fetch_prim<false>(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0), q);
+    rho[n] = q.rho; vel[n][0] = q.u; vel[n][1] = q.v; vel[n][2] = q.w;
+    derive_pH(P, q, pp[n], Hh[n]);
+    cs[n] = sqrt(P.gam * P.Rgas * q.T);
+  }
+  // central flux, flux form of Eq. 7: pairs (i-m, i-m+l); local index of node i is 2
+  double Fc[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+  for (int l = 1; l <= 3; ++l) {
+    const double a = P.c.a[l - 1];
+#pragma unroll
+    for (int m = 0; m < l; ++m) {
+      const int ia = 2 - m, ib = 2 - m + l;
+      const double mm = (rho[ia] + rho[ib]) * (vel[ia][D] + vel[ib][D]);
+      Fc[0] += (0.5 * a) * mm;
+      Fc[1] += (0.25 * a) * (mm * (vel[ia][0] + vel[ib][0]));
+      Fc[2] += (0.25 * a) * (mm * (vel[ia][1] + vel[ib][1]));
+      Fc[3] += (0.25 * a) * (mm * (vel[ia][2] + vel[ib][2]));
+      Fc[4] += (0.25 * a) * (mm * (Hh[ia] + Hh[ib]));
+      Fc[1 + D] += a * (pp[ia] + pp[ib]);
+    }
+  }
+  // Roe state (S6 step 1) and eigenvectors (step 2)
+  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
+  const double r = sqrt(rho[3] / rho[2]), ir1 = 1.0 / (1.0 + r);
+  double ub[3];
+#pragma unroll
+  for (int m = 0; m < 3; ++m) ub[m] = (vel[2][m] + r * vel[3][m]) * ir1;
+  const double Hb = (Hh[2] + r * Hh[3]) * ir1;
+  const double q2 = ub[0] * ub[0] + ub[1] * ub[1] + ub[2] * ub[2];
+  const double c2 = P.gm1 * (Hb - 0.5 * q2), cb = sqrt(c2), icb = 1.0 / cb;
+  const double b1 = P.gm1 / c2, b2 = 0.5 * q2 * b1;
+  const double un = ub[D];
+  // steps 3-4: characteristic variables/fluxes at the six nodes, local LF speeds
+  double wc[6][5], fc[6][5], al[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+  for (int n = 0; n < 6; ++n) {
+    const double vn = vel[n][D];
+    const double wv[5] = {rho[n], rho[n] * vel[n][0], rho[n] * vel[n][1], rho[n] * vel[n][2], rho[n] * Hh[n] - pp[n]};
+    double fv[5] = {rho[n] * vn, wv[1] * vn, wv[2] * vn, wv[3] * vn, rho[n] * vn * Hh[n]};
+    fv[1 + D] += pp[n];
+    const double mw = ub[0] * wv[1] + ub[1] * wv[2] + ub[2] * wv[3];
+    const double mf = ub[0] * fv[1] + ub[1] * fv[2] + ub[2] * fv[3];
+    wc[n][0] = 0.5 * ((b2 + un * icb) * wv[0] - b1 * mw - wv[1 + D] * icb + b1 * wv[4]);
+    fc[n][0] = 0.5 * ((b2 + un * icb) * fv[0] - b1 * mf - fv[1 + D] * icb + b1 * fv[4]);
+    wc[n][1] = (1.0 - b2) * wv[0] + b1 * mw - b1 * wv[4];
+    fc[n][1] = (1.0 - b2) * fv[0] + b1 * mf - b1 * fv[4];
+    wc[n][2] = -ub[T1] * wv[0] + wv[1 + T1];
+    fc[n][2] = -ub[T1] * fv[0] + fv[1 + T1];
+    wc[n][3] = -ub[T2] * wv[0] + wv[1 + T2];
+    fc[n][3] = -ub[T2] * fv[0] + fv[1 + T2];
+    wc[n][4] = 0.5 * ((b2 - un * icb) * wv[0] - b1 * mw + wv[1 + D] * icb + b1 * wv[4]);
+    fc[n][4] = 0.5 * ((b2 - un * icb) * fv[0] - b1 * mf + fv[1 + D] * icb + b1 * fv[4]);
+    al[0] = fmax(al[0], fabs(vn - cs[n]));
+    al[1] = fmax(al[1], fabs(vn));
+    al[4] = fmax(al[4], fabs(vn + cs[n]));
+  }
+  al[2] = al[1]; al[3] = al[1];
+  // steps 5-6: split and reconstruct
+  double fh[5];
+#pragma unroll
+  for (int s = 0; s < 5; ++s) {
+    double fp[6], fm[6];
+#pragma unroll
+    for (int n = 0; n < 6; ++n) { fp[n] = 0.5 * (fc[n][s] + al[s] * wc[n][s]); fm[n] = 0.5 * (fc[n][s] - al[s] * wc[n][s]); }
+    fh[s] = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+  }
+  // step 7: back to conservative variables
+  double Fw[5];
+  Fw[0] = fh[0] + fh[1] + fh[4];
+#pragma unroll
+  for (int m = 0; m < 3; ++m) Fw[1 + m] = ub[m] * (fh[0] + fh[1] + fh[4]);
+  Fw[1 + D] += cb * (fh[4] - fh[0]);
+  Fw[1 + T1] += fh[2];
+  Fw[1 + T2] += fh[3];
+  Fw[4] = (Hb - un * cb) * fh[0] + 0.5 * q2 * fh[1] + ub[T1] * fh[2] + ub[T2] * fh[3] + (Hb + un * cb) * fh[4];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) dF[v] = Fw[v] - Fc[v];
+}
+
+// one thread per listed node: R += dR, and (if w_new) w_new += dt beta dR  (Eq. 11 is linear in R)
+__global__ void __launch_bounds__(128) k_weno_apply(const DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
+                                                    const unsigned char* __restrict__ lmask, const DevScal* __restrict__ sc,
+                                                    double* __restrict__ R, double* __restrict__ w_new, double beta) {
+  const unsigned int n = sc->list_count;
+  const double dtb = sc->dt * beta;
+  for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+    const long long o = list[e];
+    const int mask = lmask[e];
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    double dR[5] = {0, 0, 0, 0, 0};
+    double dF[5];
+    const bool skip_x = i == P.nx - 1 && P.bc[1] == BC_OUTFLOW;   // S8 replaces the x-difference there
+    if (!skip_x) {
+      const double ih = P.ih[0][i];
+      if (mask & 1) { weno_delta<0>(P, w, i - 1, j, k, dF);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dR[v] += ih * dF[v]; }
+      if (mask & 2) { weno_delta<0>(P, w, i, j, k, dF);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dR[v] -= ih * dF[v]; }
+    }
+    {
+      const double ih = P.ih[1][j];
+      if (mask & 4) { weno_delta<1>(P, w, i, j - 1, k, dF);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dR[v] += ih * dF[v]; }
+      if (mask & 8) { weno_delta<1>(P, w, i, j, k, dF);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dR[v] -= ih * dF[v]; }
+    }
+    {
+      const double ih = P.ih[2][k];
+      if (mask & 16) { weno_delta<2>(P, w, i, j, k - 1, dF);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dR[v] += ih * dF[v]; }
+      if (mask & 32) { weno_delta<2>(P, w, i, j, k, dF);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dR[v] -= ih * dF[v]; }
+    }
+#pragma unroll
+    for (int v = 0; v < 5; ++v) R[o + v * P.N] += dR[v];
+    if (w_new) {
+      const bool wall = (j == 0 && P.bc[2] == BC_WALL_NODE) || (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE);
+      if (wall) {
+        const double rn = w_new[o] + dtb * dR[0];
+        w_new[o] = rn;
+        w_new[o + 4 * P.N] = rn * P.cv * (j == 0 ? P.Twall[0] : P.Twall[1]);
+      } else {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) w_new[o + v * P.N] += dtb * dR[v];
+      }
+    }
+  }
+}
+
+}  // namespace streams

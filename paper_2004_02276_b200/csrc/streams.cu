@@ -1,0 +1,541 @@
+// streams.cu -- C-ABI entry points of include/streams.h: context, metrics, launch sequence.
+//
+// Host logic only: every field-sized operation is a kernel from k_rhs.cuh / k_aux.cuh /
+// k_weno.cuh enqueued on the caller's stream.  There is no CPU fallback: any CUDA failure
+// is reported as STREAMS_ECUDA.
+#include "../../include/streams.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dev_common.cuh"
+#include "k_aux.cuh"
+#include "k_rhs.cuh"
+#include "k_weno.cuh"
+
+using namespace streams;
+
+namespace {
+thread_local char g_err[256] = "no error";
+constexpr int RGRID = 148 * 8;           // CTAs of the grid-stride reduction kernels (148 SMs)
+constexpr size_t ALIGN = 256;
+inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+}  // namespace
+
+struct streams_ctx {
+  streams_grid g;
+  streams_params p;
+  DevP P;
+  cudaStream_t st;
+  // workspace carve-up (caller memory)
+  double *wbuf[2], *S[2], *theta, *partial, *inflow, *speeds;
+  unsigned char *nflag, *lmask;
+  unsigned int* list;
+  int npartial;
+  // context-owned small device memory
+  void* small_dev;
+  DevScal* sc;
+  int cur, scur;                 // current state buffer, current "previous-R" buffer
+  int has_state;
+  long long step;
+  long long launches;
+  dim3 rhs_grid;
+  int lz;
+  char err[256];
+};
+
+namespace {
+
+int fail(streams_ctx* c, int code, const char* msg) {
+  snprintf(g_err, sizeof g_err, "%s", msg);
+  if (c) snprintf(c->err, sizeof c->err, "%s", msg);
+  return code;
+}
+int cuda_fail(streams_ctx* c, cudaError_t e, const char* where) {
+  char b[256];
+  snprintf(b, sizeof b, "CUDA error at %s: %s", where, cudaGetErrorString(e));
+  return fail(c, STREAMS_ECUDA, b);
+}
+#define CK(call)                                                   \
+  do {                                                             \
+    cudaError_t e_ = (call);                                       \
+    if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);         \
+  } while (0)
+#define LAUNCH_CHECK(name)                                         \
+  do {                                                             \
+    c->launches++;                                                 \
+    cudaError_t e_ = cudaGetLastError();                           \
+    if (e_ != cudaSuccess) return cuda_fail(c, e_, name);          \
+  } while (0)
+
+bool coeffs(int order, Coef& k) {
+  for (int i = 0; i < 3; ++i) k.a[i] = k.b[i] = 0.0;
+  if (order == 2) { k.a[0] = 0.5; k.b[0] = 1.0; return true; }
+  if (order == 4) { k.a[0] = 2.0 / 3.0; k.a[1] = -1.0 / 12.0; k.b[0] = 4.0 / 3.0; k.b[1] = -1.0 / 12.0; return true; }
+  if (order == 6) { k.a[0] = 0.75; k.a[1] = -0.15; k.a[2] = 1.0 / 60.0; k.b[0] = 1.5; k.b[1] = -0.15; k.b[2] = 1.0 / 90.0; return true; }
+  return false;
+}
+
+const char* validate(const streams_grid* g, const streams_params* p) {
+  if (g->nx < 1 || g->ny < 1 || g->nz < 1) return "grid sizes must be >= 1";
+  if ((long long)g->nx * g->ny * g->nz > 0xffffffffLL) return "more than 2^32 nodes";
+  if (!(p->gamma > 1.0) || !(p->Rgas > 0.0) || !(p->Pr > 0.0)) return "gamma > 1, Rgas > 0, Pr > 0 required";
+  if (p->order != 2 && p->order != 4 && p->order != 6) return "order must be 2, 4 or 6";
+  if (p->weno_enable && !(p->sensor_eps > 0.0)) return "sensor_eps must be > 0 (Eq. 8 is 0/0 in uniform flow otherwise)";
+  if (p->visc_model != STREAMS_VISC_POWER && p->visc_model != STREAMS_VISC_SUTHERLAND) return "unknown visc_model";
+  if (!(p->cfl > 0.0) && !(p->dt_fixed > 0.0)) return "cfl > 0 or dt_fixed > 0 required";
+  const int n[3] = {g->nx, g->ny, g->nz};
+  for (int d = 0; d < 3; ++d) {
+    const int lo = p->bc[2 * d], hi = p->bc[2 * d + 1];
+    if ((lo == STREAMS_BC_PERIODIC) != (hi == STREAMS_BC_PERIODIC)) return "periodic must be set on both faces of a direction";
+    if (lo != STREAMS_BC_PERIODIC && n[d] < 4) return "non-periodic directions need >= 4 nodes";
+    if (lo == STREAMS_BC_PERIODIC && !(g->len[d] > 0.0)) return "periodic directions need len > 0";
+    for (int s = 0; s < 2; ++s) {
+      const int b = p->bc[2 * d + s];
+      if (b < 0 || b > STREAMS_BC_EXTRAP) return "unknown boundary kind";
+      if ((b == STREAMS_BC_WALL_ISO_STAGGERED || b == STREAMS_BC_WALL_ISO_NODE) && d != 1) return "walls are supported on y faces only";
+      if (b == STREAMS_BC_INFLOW_FROZEN && !(d == 0 && s == 0)) return "INFLOW_FROZEN is supported on xmin only";
+      if (b == STREAMS_BC_OUTFLOW_NR && !(d == 0 && s == 1)) return "OUTFLOW_NR is supported on xmax only";
+      if (b == STREAMS_BC_SHOCKGEN && !(d == 1 && s == 1)) return "SHOCKGEN is supported on ymax only";
+    }
+  }
+  if (p->forcing && p->bc[0] != STREAMS_BC_PERIODIC) return "bulk forcing needs a periodic x direction";
+  return nullptr;
+}
+
+double visc_host(const streams_params& p, double T) {
+  if (p.visc_model == STREAMS_VISC_SUTHERLAND) return p.mu_ref * std::pow(T / p.T_ref, 1.5) * (p.T_ref + p.suth_S) / (T + p.suth_S);
+  return p.mu_ref * std::pow(T / p.T_ref, p.visc_exp);
+}
+
+// S1 shock generator: weak oblique-shock solution for the deflection angle
+bool shock_post_state(const streams_params& p, double post[6]) {
+  const double g = p.gamma, u1 = p.fs[1], T1 = p.fs[4];
+  const double M = u1 / std::sqrt(g * p.Rgas * T1);
+  const double tphi = std::tan(p.shock_angle_deg * 3.14159265358979323846 / 180.0);
+  if (!(M > 1.0) || !(tphi > 0.0)) return false;
+  auto f = [&](double b) { const double s = std::sin(b); return 2.0 / std::tan(b) * (M * M * s * s - 1.0) / (M * M * (g + std::cos(2.0 * b)) + 2.0); };
+  // golden-section search of the maximum-deflection angle, then bisection on the weak branch
+  const double mu = std::asin(1.0 / M);
+  double a = mu, b = 0.5 * 3.14159265358979323846;
+  const double gr = 0.6180339887498949;
+  for (int it = 0; it < 200; ++it) {
+    const double x1 = b - gr * (b - a), x2 = a + gr * (b - a);
+    if (f(x1) < f(x2)) a = x1; else b = x2;
+  }
+  const double bmax = 0.5 * (a + b);
+  if (f(bmax) < tphi) return false;
+  double lo = mu, hi = bmax;
+  for (int it = 0; it < 200; ++it) { const double m = 0.5 * (lo + hi); if (f(m) < tphi) lo = m; else hi = m; }
+  const double be = 0.5 * (lo + hi), sb = std::sin(be), cb = std::cos(be);
+  const double Mn = M * sb;
+  const double pr = 1.0 + 2.0 * g / (g + 1.0) * (Mn * Mn - 1.0);
+  const double rr = (g + 1.0) * Mn * Mn / ((g - 1.0) * Mn * Mn + 2.0);
+  const double ut = u1 * cb, un2 = u1 * sb / rr;
+  post[0] = p.fs[0] * rr;
+  post[1] = ut * cb + un2 * sb;
+  post[2] = -ut * sb + un2 * cb;
+  post[3] = p.fs[3];
+  post[4] = T1 * pr / rr;
+  post[5] = visc_host(p, post[4]);
+  return true;
+}
+
+struct Carve { size_t off = 0; size_t take(size_t bytes) { size_t o = off; off += up(bytes); return o; } };
+
+struct Layout { size_t w[2], S[2], theta, nflag, lmask, list, partial, inflow, speeds, total; int npartial; dim3 grid; int lz; };
+
+Layout make_layout(const streams_grid& g, const streams_params& p) {
+  Layout L;
+  const size_t N = (size_t)g.nx * g.ny * g.nz;
+  Carve c;
+  for (int i = 0; i < 2; ++i) L.w[i] = c.take(5 * N * sizeof(double));
+  for (int i = 0; i < 2; ++i) L.S[i] = c.take(5 * N * sizeof(double));
+  L.theta = L.nflag = L.lmask = L.list = 0;
+  if (p.weno_enable) {
+    L.theta = c.take(N * sizeof(double));
+    L.nflag = c.take(N);
+    L.lmask = c.take(N);
+    L.list = c.take(N * sizeof(unsigned int));
+  }
+  const int tiles_x = (g.nx + TX - 1) / TX, tiles_y = (g.ny + TY - 1) / TY;
+  const int tiles = tiles_x * tiles_y;
+  int nchunk = (2 * 148 + tiles - 1) / tiles;            // at least ~2 waves of CTAs on 148 SMs
+  nchunk = std::max(nchunk, (g.nz + 127) / 128);         // cap the chunk length
+  nchunk = std::min(nchunk, std::max(1, g.nz / 8));      // but keep the 6-plane warm-up amortised
+  L.lz = (g.nz + nchunk - 1) / nchunk;
+  nchunk = (g.nz + L.lz - 1) / L.lz;
+  L.grid = dim3(tiles_x, tiles_y, nchunk);
+  L.npartial = std::max(tiles * nchunk, NDIAG * RGRID);
+  L.partial = c.take((size_t)L.npartial * sizeof(double));
+  L.inflow = c.take((size_t)5 * g.nz * g.ny * sizeof(double));
+  L.speeds = c.take(8 * sizeof(double));
+  L.total = c.off;
+  return L;
+}
+
+int rgrid_for(long long N) { return (int)std::min<long long>(RGRID, (N + RT - 1) / RT); }
+
+}  // namespace
+
+extern "C" {
+
+size_t streams_workspace_bytes(const streams_grid* g, const streams_params* p) {
+  if (!g || !p || validate(g, p)) return 0;
+  return make_layout(*g, *p).total;
+}
+
+const char* streams_last_error(const streams_ctx* c) { return c ? c->err : g_err; }
+
+long long streams_launch_count(const streams_ctx* c) { return c ? c->launches : 0; }
+
+void streams_destroy(streams_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->st);
+  if (c->small_dev) cudaFree(c->small_dev);
+  delete c;
+}
+
+int streams_create(const streams_grid* g, const double* hx, const double* hy, const double* hz, const streams_params* p,
+                   void* d_workspace, size_t workspace_bytes, void* cuda_stream, streams_ctx** out) {
+  streams_ctx* c = nullptr;
+  if (!g || !hx || !hy || !hz || !p || !out) return fail(nullptr, STREAMS_EINVAL, "null argument");
+  if (const char* m = validate(g, p)) return fail(nullptr, STREAMS_EINVAL, m);
+  const Layout L = make_layout(*g, *p);
+  if (!d_workspace || workspace_bytes < L.total) return fail(nullptr, STREAMS_ENOMEM, "workspace too small");
+  if (((size_t)d_workspace) % ALIGN) return fail(nullptr, STREAMS_ENOMEM, "workspace must be 256-byte aligned");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(nullptr, STREAMS_ECUDA, "no CUDA device: this library has no CPU path");
+
+  c = new (std::nothrow) streams_ctx();
+  if (!c) return fail(nullptr, STREAMS_ENOMEM, "host allocation failed");
+  std::memset(c, 0, sizeof *c);
+  snprintf(c->err, sizeof c->err, "no error");
+  c->g = *g; c->p = *p;
+  c->st = (cudaStream_t)cuda_stream;
+  char* base = (char*)d_workspace;
+  for (int i = 0; i < 2; ++i) { c->wbuf[i] = (double*)(base + L.w[i]); c->S[i] = (double*)(base + L.S[i]); }
+  if (p->weno_enable) {
+    c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
+    c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
+  }
+  c->partial = (double*)(base + L.partial); c->inflow = (double*)(base + L.inflow); c->speeds = (double*)(base + L.speeds);
+  c->npartial = L.npartial; c->rhs_grid = L.grid; c->lz = L.lz;
+
+  // ---- S1 ghost coordinates and S2 metrics (host, O(n)) ----
+  const int n[3] = {g->nx, g->ny, g->nz};
+  const double* xin[3] = {hx, hy, hz};
+  Coef K;
+  coeffs(p->order, K);
+  std::vector<double> ih[3], gh[3], hh[3], xg0;
+  double voltot_dir[3];
+  for (int d = 0; d < 3; ++d) {
+    for (int i = 1; i < n[d]; ++i)
+      if (!(xin[d][i] > xin[d][i - 1])) { delete c; return fail(nullptr, STREAMS_EINVAL, "coordinates must be strictly increasing"); }
+    std::vector<double> xc(n[d] + 2 * HALO);
+    for (int i = 0; i < n[d]; ++i) xc[i + HALO] = xin[d][i];
+    for (int l = 1; l <= HALO; ++l)
+      for (int s = 0; s < 2; ++s) {
+        const int gi = s == 0 ? -l : n[d] - 1 + l;
+        const int bc = p->bc[2 * d + s];
+        double v;
+        if (bc == STREAMS_BC_PERIODIC) {
+          int r = gi % n[d]; if (r < 0) r += n[d];
+          v = xin[d][r] + (double)((gi - r) / n[d]) * g->len[d];
+        } else if (bc == STREAMS_BC_WALL_ISO_STAGGERED) {
+          v = 2.0 * p->y_wall[s] - xin[d][s == 0 ? l - 1 : n[d] - l];
+        } else {
+          v = 2.0 * xin[d][s == 0 ? 0 : n[d] - 1] - xin[d][s == 0 ? l : n[d] - 1 - l];
+        }
+        xc[gi + HALO] = v;
+      }
+    ih[d].resize(n[d]); gh[d].resize(n[d]); hh[d].resize(n[d]);
+    double tot = 0.0;
+    for (int i = 0; i < n[d]; ++i) {
+      double h = 0.0, gg = 0.0;
+      for (int l = 1; l <= 3; ++l) {
+        h += K.a[l - 1] * (xc[i + HALO + l] - xc[i + HALO - l]);
+        gg += K.b[l - 1] * ((xc[i + HALO + l] - xc[i + HALO]) - (xc[i + HALO] - xc[i + HALO - l]));
+      }
+      if (!(h > 0.0)) { delete c; return fail(nullptr, STREAMS_EINVAL, "non-positive metric"); }
+      hh[d][i] = h; ih[d][i] = 1.0 / h; gh[d][i] = -gg / (h * h * h);
+      tot += h;
+    }
+    voltot_dir[d] = tot;
+    if (d == 0) xg0 = xc;
+  }
+  // total volume: sum over nodes of hx hy hz, summed the same way a serial loop would (used only as a divisor)
+  double voltot = 0.0;
+  for (int k = 0; k < n[2]; ++k)
+    for (int j = 0; j < n[1]; ++j) voltot += voltot_dir[0] * hh[1][j] * hh[2][k];
+
+  // ---- device parameter block ----
+  DevP& P = c->P;
+  P.nx = n[0]; P.ny = n[1]; P.nz = n[2]; P.N = (long long)n[0] * n[1] * n[2];
+  for (int i = 0; i < 6; ++i) P.bc[i] = p->bc[i];
+  P.visc_model = p->visc_model; P.weno = p->weno_enable; P.forcing = p->forcing; P.viscous = p->viscous_enable; P.L = p->order / 2;
+  P.gam = p->gamma; P.gm1 = p->gamma - 1.0; P.Rgas = p->Rgas; P.inv_R = 1.0 / p->Rgas;
+  P.cp = p->gamma * p->Rgas / (p->gamma - 1.0); P.cv = p->Rgas / (p->gamma - 1.0); P.cp_over_Pr = P.cp / p->Pr;
+  P.mu_ref = p->mu_ref; P.T_ref = p->T_ref; P.inv_Tref = 1.0 / p->T_ref; P.visc_exp = p->visc_exp; P.suth_S = p->suth_S;
+  P.th_thr = p->sensor_threshold; P.th_eps = p->sensor_eps;
+  P.Twall[0] = p->T_wall[0]; P.Twall[1] = p->T_wall[1];
+  P.c = K;
+  for (int i = 0; i < 5; ++i) P.fs[i] = p->fs[i];
+  P.fs[5] = visc_host(*p, p->fs[4]);
+  for (int i = 0; i < 6; ++i) P.post[i] = P.fs[i];
+  std::vector<unsigned char> xpost(n[0] + 2 * HALO, 0);
+  if (p->bc[3] == STREAMS_BC_SHOCKGEN) {
+    if (!shock_post_state(*p, P.post)) { delete c; return fail(nullptr, STREAMS_EINVAL, "shock generator: no attached weak shock for these parameters"); }
+    for (int i = 0; i < n[0] + 2 * HALO; ++i) xpost[i] = xg0[i] < p->x_shock ? 0 : 1;   // sharp jump (A15)
+  }
+
+  // ---- small device arrays ----
+  size_t off = 0, o_arr[9], o_xpost, o_sc;
+  for (int a = 0; a < 9; ++a) { o_arr[a] = off; off += up((size_t)n[a % 3] * sizeof(double)); }
+  o_xpost = off; off += up(xpost.size());
+  o_sc = off; off += up(sizeof(DevScal));
+  cudaError_t e = cudaMalloc(&c->small_dev, off);
+  if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(metrics)"); }
+  char* sb = (char*)c->small_dev;
+  std::vector<double>* src[9] = {&ih[0], &ih[1], &ih[2], &gh[0], &gh[1], &gh[2], &hh[0], &hh[1], &hh[2]};
+  for (int a = 0; a < 9; ++a) {
+    e = cudaMemcpyAsync(sb + o_arr[a], src[a]->data(), src[a]->size() * sizeof(double), cudaMemcpyHostToDevice, c->st);
+    if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaMemcpy(metrics)"); }
+  }
+  for (int d = 0; d < 3; ++d) { P.ih[d] = (const double*)(sb + o_arr[d]); P.gh[d] = (const double*)(sb + o_arr[3 + d]); P.hh[d] = (const double*)(sb + o_arr[6 + d]); }
+  cudaMemcpyAsync(sb + o_xpost, xpost.data(), xpost.size(), cudaMemcpyHostToDevice, c->st);
+  P.xpost = (const unsigned char*)(sb + o_xpost);
+  P.inflow = c->inflow;
+  c->sc = (DevScal*)(sb + o_sc);
+  DevScal hs;
+  std::memset(&hs, 0, sizeof hs);
+  hs.vol_total = voltot;
+  hs.dt = p->dt_fixed > 0.0 ? p->dt_fixed : 0.0;
+  cudaMemcpyAsync(c->sc, &hs, sizeof hs, cudaMemcpyHostToDevice, c->st);
+  e = cudaStreamSynchronize(c->st);     // host vectors go out of scope
+  if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "create sync"); }
+
+  e = cudaFuncSetAttribute(k_rhs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
+  if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaFuncSetAttribute(k_rhs)"); }
+  *out = c;
+  return STREAMS_OK;
+}
+
+static int after_set_state(streams_ctx* c) {
+  if (c->p.bc[0] == STREAMS_BC_INFLOW_FROZEN) {
+    k_capture_inflow<<<64, 256, 0, c->st>>>(c->P, c->wbuf[c->cur], c->inflow);
+    LAUNCH_CHECK("k_capture_inflow");
+  }
+  // keep vol_total: reset the other scalars one by one
+  CK(cudaMemsetAsync(&c->sc->force, 0, sizeof(double), c->st));
+  CK(cudaMemsetAsync(&c->sc->time, 0, sizeof(double), c->st));
+  if (!(c->p.dt_fixed > 0.0)) CK(cudaMemsetAsync(&c->sc->dt, 0, sizeof(double), c->st));
+  c->has_state = 1; c->step = 0; c->scur = 0;
+  return STREAMS_OK;
+}
+
+int streams_set_state(streams_ctx* c, const double* d_w) {
+  if (!c || !d_w) return fail(c, STREAMS_EINVAL, "null argument");
+  c->cur = 0;
+  CK(cudaMemcpyAsync(c->wbuf[0], d_w, 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+  return after_set_state(c);
+}
+int streams_set_state_host(streams_ctx* c, const double* h_w) {
+  if (!c || !h_w) return fail(c, STREAMS_EINVAL, "null argument");
+  c->cur = 0;
+  CK(cudaMemcpyAsync(c->wbuf[0], h_w, 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyHostToDevice, c->st));
+  const int rc = after_set_state(c);
+  if (rc) return rc;
+  CK(cudaStreamSynchronize(c->st));
+  return STREAMS_OK;
+}
+int streams_get_state(streams_ctx* c, double* d_w) {
+  if (!c || !d_w) return fail(c, STREAMS_EINVAL, "null argument");
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  CK(cudaMemcpyAsync(d_w, c->wbuf[c->cur], 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+  return STREAMS_OK;
+}
+int streams_get_state_host(streams_ctx* c, double* h_w) {
+  if (!c || !h_w) return fail(c, STREAMS_EINVAL, "null argument");
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  CK(cudaMemcpyAsync(h_w, c->wbuf[c->cur], 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  CK(cudaStreamSynchronize(c->st));
+  return STREAMS_OK;
+}
+
+// sensor + list of nodes with flagged interfaces for the state in `w`
+static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsigned char* iflags_out, bool build_list) {
+  CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
+  const int rg = rgrid_for(c->P.N);
+  k_sensor<<<rg, RT, 0, c->st>>>(c->P, w, c->nflag, theta_out, c->sc);
+  LAUNCH_CHECK("k_sensor");
+  k_weno_list<<<rg, RT, 0, c->st>>>(c->P, c->nflag, build_list ? c->list : nullptr, c->lmask, iflags_out, c->sc);
+  LAUNCH_CHECK("k_weno_list");
+  return STREAMS_OK;
+}
+
+static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A) {
+  const size_t smem = SM_RHS_DOUBLES * sizeof(double);
+  if (fused) k_rhs<true><<<c->rhs_grid, dim3(TX, TY), smem, c->st>>>(c->P, A);
+  else k_rhs<false><<<c->rhs_grid, dim3(TX, TY), smem, c->st>>>(c->P, A);
+  LAUNCH_CHECK("k_rhs");
+  return STREAMS_OK;
+}
+
+static int force_from_partials(streams_ctx* c, const double* R, bool have_rhs_partials) {
+  int n = (int)(c->rhs_grid.x * c->rhs_grid.y * c->rhs_grid.z);
+  if (!have_rhs_partials) {
+    n = rgrid_for(c->P.N);
+    k_force_partial<<<n, RT, 0, c->st>>>(c->P, R, c->partial);
+    LAUNCH_CHECK("k_force_partial");
+  }
+  k_force_final<<<1, RT, 0, c->st>>>(c->partial, n, c->sc);
+  LAUNCH_CHECK("k_force_final");
+  return STREAMS_OK;
+}
+
+int streams_rhs(streams_ctx* c, double* d_rhs) {
+  if (!c || !d_rhs) return fail(c, STREAMS_EINVAL, "null argument");
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  const double* w = c->wbuf[c->cur];
+  int rc;
+  if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, true))) return rc;
+  RhsArgs A;
+  std::memset(&A, 0, sizeof A);
+  A.w = w; A.out_rhs = d_rhs; A.lz = c->lz;
+  const bool partial_ok = c->p.forcing && !c->p.weno_enable;
+  A.partial = partial_ok ? c->partial : nullptr;
+  if ((rc = launch_rhs(c, false, A))) return rc;
+  if (c->p.weno_enable) {
+    k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, d_rhs, nullptr, 0.0);
+    LAUNCH_CHECK("k_weno_apply");
+  }
+  if (c->p.forcing) {
+    if ((rc = force_from_partials(c, d_rhs, partial_ok))) return rc;
+    k_apply_force<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, w, d_rhs, c->sc);
+    LAUNCH_CHECK("k_apply_force");
+  }
+  return STREAMS_OK;
+}
+
+int streams_sensor(streams_ctx* c, double* d_theta, unsigned char* d_flags) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  if (!c->p.weno_enable) return fail(c, STREAMS_EINVAL, "streams_sensor needs weno_enable = 1");
+  return run_sensor(c, c->wbuf[c->cur], d_theta, d_flags, false);
+}
+
+int streams_step(streams_ctx* c, int nsteps) {
+  if (!c || nsteps < 0) return fail(c, STREAMS_EINVAL, "bad argument");
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  static const double alpha[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};   // Eq. 11 with the sign of reading G5
+  static const double beta[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
+  const int rg = rgrid_for(c->P.N);
+  int rc;
+  for (int s = 0; s < nsteps; ++s) {
+    if (!(c->p.dt_fixed > 0.0)) {
+      k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->wbuf[c->cur], c->partial);
+      LAUNCH_CHECK("k_speed_partial");
+      k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 1);
+      LAUNCH_CHECK("k_dt_final");
+    }
+    for (int l = 0; l < 3; ++l) {
+      double* w = c->wbuf[c->cur];
+      if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, true))) return rc;
+      RhsArgs A;
+      std::memset(&A, 0, sizeof A);
+      A.w = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
+      if (c->p.forcing) {
+        // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
+        double* Sp = c->S[c->scur];
+        double* Sc = c->S[c->scur ^ 1];
+        const bool partial_ok = !c->p.weno_enable;
+        A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
+        if ((rc = launch_rhs(c, false, A))) return rc;
+        if (c->p.weno_enable) {
+          k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, Sc, nullptr, 0.0);
+          LAUNCH_CHECK("k_weno_apply");
+        }
+        if ((rc = force_from_partials(c, Sc, partial_ok))) return rc;
+        k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1);
+        LAUNCH_CHECK("k_update");
+        c->scur ^= 1;
+      } else {
+        // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
+        double* wn = c->wbuf[c->cur ^ 1];
+        A.w_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0];
+        if ((rc = launch_rhs(c, true, A))) return rc;
+        if (c->p.weno_enable) {
+          k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->S[0], wn, beta[l]);
+          LAUNCH_CHECK("k_weno_apply");
+        }
+        c->cur ^= 1;
+      }
+    }
+    k_advance_time<<<1, 1, 0, c->st>>>(c->sc);
+    LAUNCH_CHECK("k_advance_time");
+    c->step++;
+  }
+  return STREAMS_OK;
+}
+
+int streams_diagnostics(streams_ctx* c, streams_diag* out) {
+  if (!c || !out) return fail(c, STREAMS_EINVAL, "null argument");
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  std::memset(out, 0, sizeof *out);
+  const int rg = rgrid_for(c->P.N);
+  const double* w = c->wbuf[c->cur];
+  int rc;
+  // sensor statistics of the current state (interface counts as the next RHS would see them)
+  if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, false))) return rc;
+  DevScal hs;
+  CK(cudaMemcpyAsync(&hs, c->sc, sizeof hs, cudaMemcpyDeviceToHost, c->st));
+  k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, w, c->partial);
+  LAUNCH_CHECK("k_speed_partial");
+  k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, c->speeds, 0);
+  LAUNCH_CHECK("k_dt_final");
+  double sp[3];
+  CK(cudaMemcpyAsync(sp, c->speeds, sizeof sp, cudaMemcpyDeviceToHost, c->st));
+  k_diag_partial<<<rg, RT, 0, c->st>>>(c->P, w, c->partial);
+  LAUNCH_CHECK("k_diag_partial");
+  std::vector<double> part((size_t)NDIAG * rg);
+  CK(cudaMemcpyAsync(part.data(), c->partial, part.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  CK(cudaStreamSynchronize(c->st));
+  double s[7] = {0, 0, 0, 0, 0, 0, 0}, mnr = INFINITY, mnp = INFINITY, mxm = 0.0, bad = 0.0;
+  for (int a = 0; a < 7; ++a) {
+    // pairwise-free Neumaier sum over the CTA partials (fixed order)
+    double sum = 0.0, comp = 0.0;
+    for (int b = 0; b < rg; ++b) {
+      const double x = part[(size_t)a * rg + b], t = sum + x;
+      comp += std::fabs(sum) >= std::fabs(x) ? (sum - t) + x : (x - t) + sum;
+      sum = t;
+    }
+    s[a] = sum + comp;
+  }
+  for (int b = 0; b < rg; ++b) {
+    mnr = std::fmin(mnr, part[(size_t)7 * rg + b]); mnp = std::fmin(mnp, part[(size_t)8 * rg + b]);
+    mxm = std::fmax(mxm, part[(size_t)9 * rg + b]); bad = std::fmax(bad, part[(size_t)10 * rg + b]);
+  }
+  out->step = c->step; out->time = hs.time; out->dt = hs.dt; out->forcing = hs.force;
+  out->mass = s[0]; out->mom[0] = s[1]; out->mom[1] = s[2]; out->mom[2] = s[3]; out->energy = s[4]; out->kinetic = s[5];
+  out->volume = s[6]; out->bulk_rhou = s[1] / s[6];
+  out->min_rho = mnr; out->min_p = mnp; out->max_mach = mxm; out->max_theta = c->p.weno_enable ? hs.max_theta : 0.0;
+  for (int d = 0; d < 3; ++d) out->max_speed[d] = sp[d];
+  const long long n[3] = {c->P.nx, c->P.ny, c->P.nz};
+  for (int d = 0; d < 3; ++d) {
+    const bool per = c->p.bc[2 * d] == STREAMS_BC_PERIODIC;
+    out->weno_ifaces[d] = c->p.weno_enable ? (long long)hs.weno_if[d] : 0;
+    out->total_ifaces[d] = (per ? n[d] : n[d] + 1) * n[(d + 1) % 3] * n[(d + 2) % 3];
+  }
+  const bool nonfinite = bad > 0.0 || !std::isfinite(s[0]) || !std::isfinite(s[4]);
+  out->nonfinite = nonfinite ? 1 : 0;
+  if (nonfinite) return fail(c, STREAMS_ENONFINITE, "state is not physical (NaN/Inf, rho <= 0 or p <= 0)");
+  return STREAMS_OK;
+}
+
+}  // extern "C"
