@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- fp64 grid-point updates/s per RK3 step of the STREAmS hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5|3|...]
+
+A "step" is one full RK3 step (three fused RHS evaluations + updates, CFL and forcing
+reductions) of the whole grid through the C-ABI library.  The default workload is
+BASELINE.json configs[4]: the 1024x512x512 supersonic channel block (268M points), the
+configuration the metric is quoted on; it fits one B200 (43 GB workspace).
+
+N > 1: the path does not shard (north_star: one GPU, no decomposition) -> N independent
+replicas, one per rank/GPU, no data-path collective ("replicas only", scaling = weak).
+
+--impl reference: times the CPU oracle (oracle/, plain C, as it stands) on a bounded slab
+of the same workload on the host cores; rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2004_02276_b200 import workloads as W  # noqa: E402
+
+METRIC = "fp64 grid-point updates/s per RK3 step"
+UNIT = "points/s"
+PAPER_CONTEXT = "paper: 1 Tesla P100 ~ 330 Intel KNL cores (PAPER.md:11); no absolute throughput published"
+
+
+def make_workload(cfg: int, scale: float = 1.0):
+    if cfg == 5:
+        return W.config5_channel_big()
+    if cfg == 3:
+        return W.config3_channel()
+    if cfg == 1:
+        return W.config1_tgv()
+    if cfg == 2:
+        return W.config2_isotropic()
+    if cfg == 4:
+        return W.config4_sbli()
+    raise SystemExit(f"unknown config {cfg}")
+
+
+def bytes_per_point_per_launch(params) -> int:
+    """Algorithmic HBM bytes per grid point of ONE k_rhs launch."""
+    if params["forcing"]:
+        return 80            # read w (40 B) + write R (40 B); the update is a separate kernel
+    # fused RK stage: read w, write w', read S (stages 1,2), write S (the last stage's S write is dead but done)
+    return 160
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)["hbm_gbs"], "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(wl, steps: int, planes: int = 8):
+    """Time the CPU oracle, as it stands, on a z-slab of the workload (periodic in z)."""
+    from oracle import binding as ob
+    sub = wl.slab(0, planes, halo=0, keep_forcing=True)
+    o = ob.Oracle(sub.grid, sub.x, sub.y, sub.z, sub.params)
+    o.set_state(sub.state())
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    npts = sub.npoints
+    d = o.diagnostics(check=False)
+    o.close()
+    return dict(value=npts * steps / dt, seconds=dt, cores=ob.threads(), points=npts, steps=steps,
+                sample=f"{steps} RK3 step(s) of the oracle on a {sub.grid['nx']}x{sub.grid['ny']}x{sub.grid['nz']} "
+                       f"z-slab (periodic in z) of the workload, OpenMP threads={ob.threads()}", nonfinite=int(d.nonfinite))
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    wl = make_workload(args.config)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(wl, 1, planes=4)
+    vals = []
+    t_all = 0.0
+    res = None
+    for _ in range(args.steps):
+        res = oracle_sample(wl, 1, planes=args.ref_planes)
+        vals.append(res["value"])
+        t_all += res["seconds"]
+    value = res["points"] * args.steps / t_all
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * t_all / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": wl.name, "grid": [wl.grid["nx"], wl.grid["ny"], wl.grid["nz"]],
+                      "note": "each step = one oracle RK3 step on a bounded z-slab sample"},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": res["cores"], "kind": "oracle", "sample": res["sample"]},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0, "context": PAPER_CONTEXT}
+    print(json.dumps(out), flush=True)
+
+
+def upload_state(torch, wl, dev, planes=16):
+    """Generate the seeded initial state slab by slab on the host and place it in HBM."""
+    w = torch.empty(wl.shape, dtype=torch.float64, device=dev)
+    nz = wl.grid["nz"]
+    for k0 in range(0, nz, planes):
+        k1 = min(nz, k0 + planes)
+        w[:, k0:k1].copy_(torch.from_numpy(wl.state(k0, k1)))
+    return w
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2004_02276_b200 import replicas
+    from paper_2004_02276_b200.binding import Streams, lib
+
+    lib()                                      # fail loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = make_workload(args.config)
+    npts = wl.npoints
+    s = Streams(wl.grid, wl.x, wl.y, wl.z, wl.params, device=dev)
+    w0 = upload_state(torch, wl, dev)
+    s.set_state(w0)
+    state_bytes = 5 * npts * 8
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident throughput ---------------------------------------------------------
+    s.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = s.launch_count()
+    s.profile(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    s.step(args.steps)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    rhs_ms, rhs_n = s.profile_read()
+    s.profile(False)
+    launches = s.launch_count() - launches0
+    clocks = sampler.stop()
+    ms_max = 1e3 * replicas.max_over_ranks(ms * 1e-3, dev)
+    value = replicas.aggregate_throughput(npts, args.steps, ms * 1e-3, dev)
+    diag = s.diagnostics(check=False)
+
+    # ---- end to end through the C-ABI with HOST buffers ----------------------------------
+    e2e = None
+    if not args.no_e2e:
+        try:
+            hbuf = torch.empty(wl.shape, dtype=torch.float64, pin_memory=True)
+            pinned = True
+        except Exception:
+            hbuf = torch.empty(wl.shape, dtype=torch.float64)
+            pinned = False
+        s.get_state_host_ptr(hbuf.data_ptr())
+        ksteps = max(1, min(args.steps, args.e2e_steps))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ksteps):
+            s.set_state_host_ptr(hbuf.data_ptr())      # H2D of the step's input (synchronises)
+            s.step(1)
+            s.get_state_host_ptr(hbuf.data_ptr())      # D2H of the step's result (synchronises)
+        torch.cuda.synchronize(dev)
+        te = time.perf_counter() - t0
+        e2e = {"value": replicas.aggregate_throughput(npts, ksteps, te, dev), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+               "d2h_bytes_per_step": state_bytes, "steps": ksteps, "pinned": pinned}
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        bpp = bytes_per_point_per_launch(wl.params)
+        rhs_avg_ms = rhs_ms / max(rhs_n, 1)
+        achieved = bpp * npts / (rhs_avg_ms * 1e-3) / 1e9
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "k_rhs_traffic.json")
+        if os.path.exists(tpath):
+            with open(tpath) as f:
+                traffic = json.load(f).get(wl.name)
+        step_bytes = {True: 3 * (80 + 176) + 40, False: 3 * 160 + 40}[bool(wl.params["forcing"])]
+        cpu = None
+        if not args.no_cpu:
+            r = oracle_sample(wl, 1, planes=args.ref_planes)
+            cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+               "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f64", "data": "synthetic",
+               "config": {"workload": wl.name, "grid": [wl.grid["nx"], wl.grid["ny"], wl.grid["nz"]], "points": npts,
+                          "order": wl.params["order"], "forcing": wl.params["forcing"], "weno": wl.params["weno_enable"],
+                          "parallelism": "replicas only" if world > 1 else "1 GPU",
+                          "l2": "state (10.7 GB) and RK register larger than the 126 MB L2; no flush needed"
+                          if state_bytes > 2 * 126e6 else "inputs smaller than L2 (launch-latency regime)"},
+               "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+               "roofline": {"bound": "hbm", "kernel": "k_rhs", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                            "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                            "bytes_per_point_per_launch": bpp, "launches_timed": int(rhs_n), "avg_launch_ms": rhs_avg_ms,
+                            "share_of_step": rhs_ms / ms if ms > 0 else None,
+                            "step_algorithmic_GBps": step_bytes * npts * args.steps / (ms_max * 1e-3) / 1e9},
+               "cpu_baseline": cpu,
+               "state": {"time": diag.time, "dt": diag.dt, "min_rho": diag.min_rho, "nonfinite": int(diag.nonfinite)},
+               "context": PAPER_CONTEXT}
+        print(json.dumps(out), flush=True)
+    s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number (1-5); 5 is the metric's workload")
+    ap.add_argument("--ref-planes", type=int, default=8, help="z-planes of the oracle's bounded sample")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                          # timing rules: at least three warm-up steps
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

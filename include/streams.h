@@ -150,6 +150,13 @@ int streams_step(streams_ctx* ctx, int nsteps);
  * STREAMS_ENONFINITE (with *h_out filled) if the state is not physical. */
 int streams_diagnostics(streams_ctx* ctx, streams_diag* h_out);
 
+/* Kernel timing for roofline accounting.  streams_profile(ctx, 1) clears the record and makes
+ * every following launch of the fused RHS kernel (k_rhs) be bracketed by CUDA events on the
+ * context stream; streams_profile(ctx, 0) stops.  streams_profile_read synchronises and returns
+ * the summed device time in ms and the number of k_rhs launches recorded (at most 4096). */
+int streams_profile(streams_ctx* ctx, int enable);
+int streams_profile_read(streams_ctx* ctx, double* h_ms_total, long long* h_launches);
+
 /* Number of kernel launches enqueued by this context so far (for bench accounting). */
 long long streams_launch_count(const streams_ctx* ctx);
 

@@ -16,7 +16,7 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, S
 
 EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
-           "streams_diagnostics", "streams_launch_count", "streams_last_error", "streams_destroy"]
+           "streams_diagnostics", "streams_profile", "streams_profile_read", "streams_launch_count", "streams_last_error", "streams_destroy"]
 
 
 class StreamsGrid(C.Structure):
@@ -72,6 +72,8 @@ def lib():
         L.streams_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.streams_step.argtypes = [C.c_void_p, C.c_int]
         L.streams_diagnostics.argtypes = [C.c_void_p, C.POINTER(StreamsDiag)]
+        L.streams_profile.argtypes = [C.c_void_p, C.c_int]
+        L.streams_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.streams_launch_count.argtypes = [C.c_void_p]
         L.streams_launch_count.restype = C.c_longlong
         L.streams_last_error.argtypes = [C.c_void_p]
@@ -215,6 +217,15 @@ class Streams:
         rc = lib().streams_diagnostics(self._h, C.byref(d))
         self._chk(rc, allow=() if check else (STREAMS_ENONFINITE,))
         return d
+
+    def profile(self, enable=True):
+        self._chk(lib().streams_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """(summed k_rhs device time in ms, number of k_rhs launches recorded)"""
+        ms, n = C.c_double(0.0), C.c_longlong(0)
+        self._chk(lib().streams_profile_read(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     def launch_count(self):
         return lib().streams_launch_count(self._h)

@@ -2,7 +2,7 @@
 //
 // No ghost node is ever stored: every kernel asks `fetch_*` for node (i,j,k) with indices in
 // [-3, n+3) and the boundary kind decides where the value comes from (S1; PAPER.md:110,
-// 126, 146).  The composition order x -> y -> z of the oracle's ghost fill is reproduced by
+// 126, 146).  The composition order x -> y -> z of the ghost rules (S1) is reproduced by
 // resolving z first, then y, then x (each later direction reads the earlier one's ghost).
 #pragma once
 #include <cuda_runtime.h>

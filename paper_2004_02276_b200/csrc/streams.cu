@@ -45,6 +45,8 @@ struct streams_ctx {
   long long launches;
   dim3 rhs_grid;
   int lz;
+  int prof_on, prof_n;
+  std::vector<cudaEvent_t>* prof_ev;   // pairs (start, stop) around k_rhs
   char err[256];
 };
 
@@ -197,7 +199,32 @@ void streams_destroy(streams_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->st);
   if (c->small_dev) cudaFree(c->small_dev);
+  if (c->prof_ev) { for (cudaEvent_t e : *c->prof_ev) cudaEventDestroy(e); delete c->prof_ev; }
   delete c;
+}
+
+int streams_profile(streams_ctx* c, int enable) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  if (enable && !c->prof_ev) {
+    c->prof_ev = new std::vector<cudaEvent_t>(2 * 4096);
+    for (cudaEvent_t& e : *c->prof_ev) CK(cudaEventCreate(&e));
+  }
+  if (enable) c->prof_n = 0;
+  c->prof_on = enable ? 1 : 0;
+  return STREAMS_OK;
+}
+
+int streams_profile_read(streams_ctx* c, double* ms_total, long long* launches) {
+  if (!c || !ms_total || !launches) return fail(c, STREAMS_EINVAL, "null argument");
+  CK(cudaStreamSynchronize(c->st));
+  double tot = 0.0;
+  for (int i = 0; i < c->prof_n; ++i) {
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, (*c->prof_ev)[2 * i], (*c->prof_ev)[2 * i + 1]));
+    tot += ms;
+  }
+  *ms_total = tot; *launches = c->prof_n;
+  return STREAMS_OK;
 }
 
 int streams_create(const streams_grid* g, const double* hx, const double* hy, const double* hz, const streams_params* p,
@@ -381,9 +408,12 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
 
 static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A) {
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
+  const bool rec = c->prof_on && c->prof_n < 4096;
+  if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
   if (fused) k_rhs<true><<<c->rhs_grid, dim3(TX, TY), smem, c->st>>>(c->P, A);
   else k_rhs<false><<<c->rhs_grid, dim3(TX, TY), smem, c->st>>>(c->P, A);
   LAUNCH_CHECK("k_rhs");
+  if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
 }
 

@@ -55,9 +55,10 @@ class Workload:
         """Initial conservative state for z-planes [k0, k1)."""
         return self.state_fn(k0, self.grid["nz"] if k1 is None else k1)
 
-    def slab(self, k0, k1, halo=3):
+    def slab(self, k0, k1, halo=3, keep_forcing=False):
         """A sub-workload holding planes [k0-halo, k1+halo) (periodic wrap in z): the oracle's
-        RHS on its middle planes equals the full problem's (every stencil has z-radius 3)."""
+        RHS on its middle planes equals the full problem's (every stencil has z-radius 3).
+        Forcing is a global reduction, so it is switched off unless keep_forcing."""
         nz = self.grid["nz"]
         ks = [(k % nz) for k in range(k0 - halo, k1 + halo)]
         g = dict(self.grid)
@@ -69,7 +70,8 @@ class Workload:
         parts = [self.state_fn(k, k + 1) for k in ks]
         w = np.concatenate(parts, axis=1)
         p = dict(self.params)
-        p["forcing"] = 0
+        if not keep_forcing:
+            p["forcing"] = 0
         sub = Workload(self.name + f"_slab{k0}_{k1}", g, self.x, self.y, zz, p, 0, self.seed,
                        state_fn=lambda a, b, w=w: w[:, a:b].copy())
         return sub
