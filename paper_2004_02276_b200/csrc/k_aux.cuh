@@ -1,10 +1,10 @@
-// k_aux.cuh -- RK3 update (a9), CFL reduction (a10), forcing reduction (a7), diagnostics.
+// k_aux.cuh -- state conversion (a2), RK3 update with forcing (a7, a9), CFL reduction (a10), diagnostics.
 #pragma once
 #include "dev_common.cuh"
 
 namespace streams {
 
-constexpr int RT = 256;                 // threads of the reduction kernels
+constexpr int RT = 256;                 // threads of the light grid-stride kernels
 
 // device scalars kept between kernels (no host round trip inside streams_step)
 struct DevScal {
@@ -18,44 +18,64 @@ struct DevScal {
   unsigned int pad;
 };
 
-// ---- S11: w <- w + dt (alpha R_prev + beta R), Eq. 11, with the body force of S9 ----
-__global__ void __launch_bounds__(RT) k_update(const DevP P, double* __restrict__ w, const double* __restrict__ Sp,
-                                               double* __restrict__ Sc, const DevScal* __restrict__ sc,
-                                               double alpha, double beta, int use_force) {
-  const double dt = sc->dt;
-  const double f = use_force ? sc->force : 0.0;
+// ---- S3: conservative w[5][N] -> primitives Q[6][N]  (streams_set_state) ----
+__global__ void __launch_bounds__(RT) k_cons2prim(const DevP P, const double* __restrict__ w, double* __restrict__ Q) {
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    double wv[5], r[5];
-#pragma unroll
-    for (int v = 0; v < 5; ++v) { wv[v] = w[o + v * P.N]; r[v] = Sc[o + v * P.N]; }
-    if (use_force) {
-      const double u = wv[1] / wv[0];
-      r[1] += f; r[4] += f * u;                      // Eq. 1b-c: f delta_i1 and f u_1
-      Sc[o + 1 * P.N] = r[1]; Sc[o + 4 * P.N] = r[4];
-    }
-#pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      const double sp = alpha != 0.0 ? Sp[o + v * P.N] : 0.0;
-      wv[v] += dt * (alpha * sp + beta * r[v]);
-    }
-    const int j = (int)((o / P.nx) % P.ny);
-    if ((j == 0 && P.bc[2] == BC_WALL_NODE) || (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE)) {
-      const double Twl = j == 0 ? P.Twall[0] : P.Twall[1];
-      wv[1] = 0.0; wv[2] = 0.0; wv[3] = 0.0; wv[4] = wv[0] * P.cv * Twl;
-    }
+    Prim q;
+    cons2prim(P, w[o], w[o + P.N], w[o + 2 * P.N], w[o + 3 * P.N], w[o + 4 * P.N], q);
+    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu;
+  }
+}
+// ---- primitives -> conservative (streams_get_state) ----
+__global__ void __launch_bounds__(RT) k_prim2cons(const DevP P, const double* __restrict__ Q, double* __restrict__ w) {
+  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
+    Prim q;
+    q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
+    double wv[5];
+    prim2cons(P, q, wv);
 #pragma unroll
     for (int v = 0; v < 5; ++v) w[o + v * P.N] = wv[v];
   }
 }
 
+// ---- S11 with S9: R += f (0,1,0,0,u);  w <- w + dt (alpha R_prev + beta R), Eq. 11, state kept
+// as primitives.  `keep_R` != 0 writes the two forced components of R back (the next stage reads them as R_prev).
+__global__ void __launch_bounds__(RT) k_update(const DevP P, double* __restrict__ Q, const double* __restrict__ Sp,
+                                               double* __restrict__ Sc, const DevScal* __restrict__ sc,
+                                               double alpha, double beta, int use_force, int keep_R) {
+  const double dt = sc->dt;
+  const double f = use_force ? sc->force : 0.0;
+  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
+    Prim q;
+    q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
+    double r[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) r[v] = Sc[o + v * P.N];
+    if (use_force) {
+      r[1] += f; r[4] = fma(f, q.u, r[4]);           // Eq. 1b-c: f delta_i1 and f u_1
+      if (keep_R) { Sc[o + 1 * P.N] = r[1]; Sc[o + 4 * P.N] = r[4]; }
+    }
+    double dW[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      const double sp = alpha != 0.0 ? Sp[o + v * P.N] : 0.0;
+      dW[v] = dt * (alpha * sp + beta * r[v]);
+    }
+    advance_prim(P, q, dW);
+    const int j = (int)((o / P.nx) % P.ny);
+    if (j == 0 && P.bc[2] == BC_WALL_NODE) wall_node_override(P, P.Twall[0], P.mu_wall[0], q);
+    if (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE) wall_node_override(P, P.Twall[1], P.mu_wall[1], q);
+    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu;
+  }
+}
+
 // R_rhou += f, R_rhoE += f u  (streams_rhs with forcing)
-__global__ void __launch_bounds__(RT) k_apply_force(const DevP P, const double* __restrict__ w, double* __restrict__ R,
+__global__ void __launch_bounds__(RT) k_apply_force(const DevP P, const double* __restrict__ Q, double* __restrict__ R,
                                                     const DevScal* __restrict__ sc) {
   const double f = sc->force;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const double u = w[o + P.N] / w[o];
     R[o + 1 * P.N] += f;
-    R[o + 4 * P.N] += f * u;
+    R[o + 4 * P.N] = fma(f, Q[o + P.N], R[o + 4 * P.N]);
   }
 }
 
@@ -64,7 +84,7 @@ __global__ void __launch_bounds__(RT) k_force_partial(const DevP P, const double
   __shared__ double sh[RT / 32];
   double acc = 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
     acc += R[o + P.N] * (P.hh[0][i] * P.hh[1][j] * P.hh[2][k]);
   }
   const double t = block_sum<RT>(acc, sh, threadIdx.x);
@@ -80,17 +100,15 @@ __global__ void __launch_bounds__(RT) k_force_final(const double* __restrict__ p
 }
 
 // ---- S10: dt = cfl / max_d max_nodes (|u_d| + c) / h_d ----
-__global__ void __launch_bounds__(RT) k_speed_partial(const DevP P, const double* __restrict__ w, double* __restrict__ partial /*[3][grid]*/) {
+__global__ void __launch_bounds__(RT) k_speed_partial(const DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[3][grid]*/) {
   __shared__ double sh[RT / 32];
   double m[3] = {0.0, 0.0, 0.0};
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
-    Prim q;
-    cons2prim_nomu(P, w[o], w[o + P.N], w[o + 2 * P.N], w[o + 3 * P.N], w[o + 4 * P.N], q);
-    const double cs = sqrt(P.gam * P.Rgas * q.T);
-    m[0] = fmax(m[0], (fabs(q.u) + cs) * P.ih[0][i]);
-    m[1] = fmax(m[1], (fabs(q.v) + cs) * P.ih[1][j]);
-    m[2] = fmax(m[2], (fabs(q.w) + cs) * P.ih[2][k]);
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    const double cs = sqrt(P.gam * P.Rgas * Q[o + 4 * P.N]);
+    m[0] = fmax(m[0], (fabs(Q[o + P.N]) + cs) * P.ih[0][i]);
+    m[1] = fmax(m[1], (fabs(Q[o + 2 * P.N]) + cs) * P.ih[1][j]);
+    m[2] = fmax(m[2], (fabs(Q[o + 3 * P.N]) + cs) * P.ih[2][k]);
   }
   for (int d = 0; d < 3; ++d) {
     const double t = block_max<RT>(m[d], sh, threadIdx.x);
@@ -113,22 +131,24 @@ __global__ void k_advance_time(DevScal* sc) { sc->time += sc->dt; }
 
 // ---- diagnostics: per-block partials, reduced on the host by streams_diagnostics ----
 constexpr int NDIAG = 12;   // mass, mx, my, mz, E, ke, vol | min rho, min p, max Mach | nonfinite | spare
-__global__ void __launch_bounds__(RT) k_diag_partial(const DevP P, const double* __restrict__ w, double* __restrict__ partial /*[NDIAG][grid]*/) {
+__global__ void __launch_bounds__(RT) k_diag_partial(const DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[NDIAG][grid]*/) {
   __shared__ double sh[RT / 32];
   double s[7] = {0, 0, 0, 0, 0, 0, 0};
   double mnr = INFINITY, mnp = INFINITY, mxm = 0.0, bad = 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
     const double vol = P.hh[0][i] * P.hh[1][j] * P.hh[2][k];
-    const double r = w[o], ru = w[o + P.N], rv = w[o + 2 * P.N], rw = w[o + 3 * P.N], rE = w[o + 4 * P.N];
     Prim q;
-    cons2prim_nomu(P, r, ru, rv, rw, rE, q);
-    const double ke = 0.5 * r * (q.u * q.u + q.v * q.v + q.w * q.w);
-    const double p = P.gm1 * (rE - ke);
-    s[0] += r * vol; s[1] += ru * vol; s[2] += rv * vol; s[3] += rw * vol; s[4] += rE * vol; s[5] += ke * vol; s[6] += vol;
-    if (!(r > 0.0) || !(p > 0.0) || !isfinite(r) || !isfinite(p) || !isfinite(rE)) bad = 1.0;
-    mnr = fmin(mnr, r); mnp = fmin(mnp, p);
-    mxm = fmax(mxm, sqrt((q.u * q.u + q.v * q.v + q.w * q.w) / (P.gam * P.Rgas * q.T)));
+    q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
+    double wv[5];
+    prim2cons(P, q, wv);
+    const double q2 = q.u * q.u + q.v * q.v + q.w * q.w;
+    const double ke = 0.5 * q.rho * q2;
+    const double p = q.rho * (P.Rgas * q.T);
+    s[0] += wv[0] * vol; s[1] += wv[1] * vol; s[2] += wv[2] * vol; s[3] += wv[3] * vol; s[4] += wv[4] * vol; s[5] += ke * vol; s[6] += vol;
+    if (!(q.rho > 0.0) || !(p > 0.0) || !isfinite(q.rho) || !isfinite(p) || !isfinite(wv[4])) bad = 1.0;
+    mnr = fmin(mnr, q.rho); mnp = fmin(mnp, p);
+    mxm = fmax(mxm, sqrt(q2 / (P.gam * P.Rgas * q.T)));
   }
   for (int a = 0; a < 7; ++a) {
     const double t = block_sum<RT>(s[a], sh, threadIdx.x);
@@ -141,13 +161,13 @@ __global__ void __launch_bounds__(RT) k_diag_partial(const DevP P, const double*
   t = block_max<RT>(bad, sh, threadIdx.x);   if (threadIdx.x == 0) partial[10 * gridDim.x + blockIdx.x] = t;
 }
 
-// capture the frozen inflow plane (S1 INFLOW_FROZEN): inflow[v][k][j] = w[v][k][j][0]
-__global__ void k_capture_inflow(const DevP P, const double* __restrict__ w, double* __restrict__ inflow) {
+// capture the frozen inflow plane (S1 INFLOW_FROZEN): inflow[v][k][j] = Q[v][k][j][0]
+__global__ void k_capture_inflow(const DevP P, const double* __restrict__ Q, double* __restrict__ inflow) {
   const long long n = (long long)P.nz * P.ny;
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < 5 * n; e += (long long)gridDim.x * blockDim.x) {
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < NQ * n; e += (long long)gridDim.x * blockDim.x) {
     const int v = (int)(e / n);
     const long long r = e % n;
-    inflow[e] = w[v * P.N + r * P.nx];
+    inflow[e] = Q[v * P.N + r * P.nx];
   }
 }
 

@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(RT) k_sensor(const DevP P, const double* __res
   __shared__ double sh[RT / 32];
   double tmax = 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
     double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(RT) k_weno_list(const DevP P, const unsigned c
                                                   unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
   unsigned long long cnt[3] = {0, 0, 0};
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
     const int id[3] = {i, j, k};
     int mask = 0;
 #pragma unroll
@@ -121,9 +121,9 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
   for (int n = 0; n < 6; ++n) {
     const int off = n - 2;
     Prim q;
-    fetch_prim<false>(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0), q);
+    fetch_prim(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0), q);
     rho[n] = q.rho; vel[n][0] = q.u; vel[n][1] = q.v; vel[n][2] = q.w;
-    derive_pH(P, q, pp[n], Hh[n]);
+    derive_pH(P, q.rho, q.u, q.v, q.w, q.T, pp[n], Hh[n]);
     cs[n] = sqrt(P.gam * P.Rgas * q.T);
   }
   // central flux, flux form of Eq. 7: pairs (i-m, i-m+l); local index of node i is 2
@@ -201,16 +201,17 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
   for (int v = 0; v < 5; ++v) dF[v] = Fw[v] - Fc[v];
 }
 
-// one thread per listed node: R += dR, and (if w_new) w_new += dt beta dR  (Eq. 11 is linear in R)
+// one thread per listed node: R += dR, and (if q_new) the node of the already advanced state takes the
+// conservative increment dt beta dR  (Eq. 11 is linear in R)
 __global__ void __launch_bounds__(128) k_weno_apply(const DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
                                                     const unsigned char* __restrict__ lmask, const DevScal* __restrict__ sc,
-                                                    double* __restrict__ R, double* __restrict__ w_new, double beta) {
+                                                    double* __restrict__ R, double* __restrict__ q_new, double beta) {
   const unsigned int n = sc->list_count;
   const double dtb = sc->dt * beta;
   for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
     const long long o = list[e];
     const int mask = lmask[e];
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / ((long long)P.nx * P.ny));
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
     double dR[5] = {0, 0, 0, 0, 0};
     double dF[5];
     const bool skip_x = i == P.nx - 1 && P.bc[1] == BC_OUTFLOW;   // S8 replaces the x-difference there
@@ -243,15 +244,18 @@ __global__ void __launch_bounds__(128) k_weno_apply(const DevP P, const double* 
     }
 #pragma unroll
     for (int v = 0; v < 5; ++v) R[o + v * P.N] += dR[v];
-    if (w_new) {
+    if (q_new) {
       const bool wall = (j == 0 && P.bc[2] == BC_WALL_NODE) || (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE);
       if (wall) {
-        const double rn = w_new[o] + dtb * dR[0];
-        w_new[o] = rn;
-        w_new[o + 4 * P.N] = rn * P.cv * (j == 0 ? P.Twall[0] : P.Twall[1]);
+        q_new[o] += dtb * dR[0];                      // u = v = w = 0 and T = T_w stay as overridden (S1)
       } else {
+        Prim q;
+        q.rho = q_new[o]; q.u = q_new[o + P.N]; q.v = q_new[o + 2 * P.N]; q.w = q_new[o + 3 * P.N]; q.T = q_new[o + 4 * P.N]; q.mu = 0.0;
+        double dW[5];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) w_new[o + v * P.N] += dtb * dR[v];
+        for (int v = 0; v < 5; ++v) dW[v] = dtb * dR[v];
+        advance_prim(P, q, dW);
+        q_new[o] = q.rho; q_new[o + P.N] = q.u; q_new[o + 2 * P.N] = q.v; q_new[o + 3 * P.N] = q.w; q_new[o + 4 * P.N] = q.T; q_new[o + 5 * P.N] = q.mu;
       }
     }
   }

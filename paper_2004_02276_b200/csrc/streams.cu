@@ -32,7 +32,7 @@ struct streams_ctx {
   DevP P;
   cudaStream_t st;
   // workspace carve-up (caller memory)
-  double *wbuf[2], *S[2], *theta, *partial, *inflow, *speeds;
+  double *qbuf[2], *S[2], *theta, *partial, *inflow, *speeds;   // qbuf: primitives [6][N]; S: R registers [5][N]
   unsigned char *nflag, *lmask;
   unsigned int* list;
   int npartial;
@@ -85,6 +85,7 @@ bool coeffs(int order, Coef& k) {
 const char* validate(const streams_grid* g, const streams_params* p) {
   if (g->nx < 1 || g->ny < 1 || g->nz < 1) return "grid sizes must be >= 1";
   if ((long long)g->nx * g->ny * g->nz > 0xffffffffLL) return "more than 2^32 nodes";
+  if ((long long)g->nx * g->ny > 0x3fffffffLL) return "more than 2^30 nodes per z-plane";
   if (!(p->gamma > 1.0) || !(p->Rgas > 0.0) || !(p->Pr > 0.0)) return "gamma > 1, Rgas > 0, Pr > 0 required";
   if (p->order != 2 && p->order != 4 && p->order != 6) return "order must be 2, 4 or 6";
   if (p->weno_enable && !(p->sensor_eps > 0.0)) return "sensor_eps must be > 0 (Eq. 8 is 0/0 in uniform flow otherwise)";
@@ -155,7 +156,7 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   Layout L;
   const size_t N = (size_t)g.nx * g.ny * g.nz;
   Carve c;
-  for (int i = 0; i < 2; ++i) L.w[i] = c.take(5 * N * sizeof(double));
+  for (int i = 0; i < 2; ++i) L.w[i] = c.take(NQ * N * sizeof(double));
   for (int i = 0; i < 2; ++i) L.S[i] = c.take(5 * N * sizeof(double));
   L.theta = L.nflag = L.lmask = L.list = 0;
   if (p.weno_enable) {
@@ -174,7 +175,7 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   L.grid = dim3(tiles_x, tiles_y, nchunk);
   L.npartial = std::max(tiles * nchunk, NDIAG * RGRID);
   L.partial = c.take((size_t)L.npartial * sizeof(double));
-  L.inflow = c.take((size_t)5 * g.nz * g.ny * sizeof(double));
+  L.inflow = c.take((size_t)NQ * g.nz * g.ny * sizeof(double));
   L.speeds = c.take(8 * sizeof(double));
   L.total = c.off;
   return L;
@@ -245,7 +246,7 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   c->g = *g; c->p = *p;
   c->st = (cudaStream_t)cuda_stream;
   char* base = (char*)d_workspace;
-  for (int i = 0; i < 2; ++i) { c->wbuf[i] = (double*)(base + L.w[i]); c->S[i] = (double*)(base + L.S[i]); }
+  for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]); c->S[i] = (double*)(base + L.S[i]); }
   if (p->weno_enable) {
     c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
     c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
@@ -302,14 +303,15 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
 
   // ---- device parameter block ----
   DevP& P = c->P;
-  P.nx = n[0]; P.ny = n[1]; P.nz = n[2]; P.N = (long long)n[0] * n[1] * n[2];
+  P.nx = n[0]; P.ny = n[1]; P.nz = n[2]; P.nxy = n[0] * n[1]; P.N = (long long)n[0] * n[1] * n[2];
   for (int i = 0; i < 6; ++i) P.bc[i] = p->bc[i];
   P.visc_model = p->visc_model; P.weno = p->weno_enable; P.forcing = p->forcing; P.viscous = p->viscous_enable; P.L = p->order / 2;
   P.gam = p->gamma; P.gm1 = p->gamma - 1.0; P.Rgas = p->Rgas; P.inv_R = 1.0 / p->Rgas;
-  P.cp = p->gamma * p->Rgas / (p->gamma - 1.0); P.cv = p->Rgas / (p->gamma - 1.0); P.cp_over_Pr = P.cp / p->Pr;
+  P.cp = p->gamma * p->Rgas / (p->gamma - 1.0); P.cv = p->Rgas / (p->gamma - 1.0); P.inv_cv = 1.0 / P.cv; P.cp_over_Pr = P.cp / p->Pr;
   P.mu_ref = p->mu_ref; P.T_ref = p->T_ref; P.inv_Tref = 1.0 / p->T_ref; P.visc_exp = p->visc_exp; P.suth_S = p->suth_S;
   P.th_thr = p->sensor_threshold; P.th_eps = p->sensor_eps;
   P.Twall[0] = p->T_wall[0]; P.Twall[1] = p->T_wall[1];
+  P.mu_wall[0] = visc_host(*p, p->T_wall[0]); P.mu_wall[1] = visc_host(*p, p->T_wall[1]);
   P.c = K;
   for (int i = 0; i < 5; ++i) P.fs[i] = p->fs[i];
   P.fs[5] = visc_host(*p, p->fs[4]);
@@ -353,9 +355,13 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   return STREAMS_OK;
 }
 
-static int after_set_state(streams_ctx* c) {
+// conservative state in d_w (device) -> primitives in qbuf[0]; captures the frozen inflow plane
+static int after_set_state(streams_ctx* c, const double* d_w) {
+  c->cur = 0;
+  k_cons2prim<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, d_w, c->qbuf[0]);
+  LAUNCH_CHECK("k_cons2prim");
   if (c->p.bc[0] == STREAMS_BC_INFLOW_FROZEN) {
-    k_capture_inflow<<<64, 256, 0, c->st>>>(c->P, c->wbuf[c->cur], c->inflow);
+    k_capture_inflow<<<64, 256, 0, c->st>>>(c->P, c->qbuf[0], c->inflow);
     LAUNCH_CHECK("k_capture_inflow");
   }
   // keep vol_total: reset the other scalars one by one
@@ -368,15 +374,13 @@ static int after_set_state(streams_ctx* c) {
 
 int streams_set_state(streams_ctx* c, const double* d_w) {
   if (!c || !d_w) return fail(c, STREAMS_EINVAL, "null argument");
-  c->cur = 0;
-  CK(cudaMemcpyAsync(c->wbuf[0], d_w, 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
-  return after_set_state(c);
+  return after_set_state(c, d_w);
 }
 int streams_set_state_host(streams_ctx* c, const double* h_w) {
   if (!c || !h_w) return fail(c, STREAMS_EINVAL, "null argument");
-  c->cur = 0;
-  CK(cudaMemcpyAsync(c->wbuf[0], h_w, 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyHostToDevice, c->st));
-  const int rc = after_set_state(c);
+  // the RK register S[1] is free between steps: it stages the conservative vector
+  CK(cudaMemcpyAsync(c->S[1], h_w, 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyHostToDevice, c->st));
+  const int rc = after_set_state(c, c->S[1]);
   if (rc) return rc;
   CK(cudaStreamSynchronize(c->st));
   return STREAMS_OK;
@@ -384,13 +388,16 @@ int streams_set_state_host(streams_ctx* c, const double* h_w) {
 int streams_get_state(streams_ctx* c, double* d_w) {
   if (!c || !d_w) return fail(c, STREAMS_EINVAL, "null argument");
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
-  CK(cudaMemcpyAsync(d_w, c->wbuf[c->cur], 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToDevice, c->st));
+  k_prim2cons<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->qbuf[c->cur], d_w);
+  LAUNCH_CHECK("k_prim2cons");
   return STREAMS_OK;
 }
 int streams_get_state_host(streams_ctx* c, double* h_w) {
   if (!c || !h_w) return fail(c, STREAMS_EINVAL, "null argument");
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
-  CK(cudaMemcpyAsync(h_w, c->wbuf[c->cur], 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  k_prim2cons<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->S[1]);
+  LAUNCH_CHECK("k_prim2cons");
+  CK(cudaMemcpyAsync(h_w, c->S[1], 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyDeviceToHost, c->st));
   CK(cudaStreamSynchronize(c->st));
   return STREAMS_OK;
 }
@@ -432,12 +439,12 @@ static int force_from_partials(streams_ctx* c, const double* R, bool have_rhs_pa
 int streams_rhs(streams_ctx* c, double* d_rhs) {
   if (!c || !d_rhs) return fail(c, STREAMS_EINVAL, "null argument");
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
-  const double* w = c->wbuf[c->cur];
+  const double* w = c->qbuf[c->cur];
   int rc;
   if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, true))) return rc;
   RhsArgs A;
   std::memset(&A, 0, sizeof A);
-  A.w = w; A.out_rhs = d_rhs; A.lz = c->lz;
+  A.q = w; A.out_rhs = d_rhs; A.lz = c->lz;
   const bool partial_ok = c->p.forcing && !c->p.weno_enable;
   A.partial = partial_ok ? c->partial : nullptr;
   if ((rc = launch_rhs(c, false, A))) return rc;
@@ -457,7 +464,7 @@ int streams_sensor(streams_ctx* c, double* d_theta, unsigned char* d_flags) {
   if (!c) return fail(c, STREAMS_EINVAL, "null argument");
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   if (!c->p.weno_enable) return fail(c, STREAMS_EINVAL, "streams_sensor needs weno_enable = 1");
-  return run_sensor(c, c->wbuf[c->cur], d_theta, d_flags, false);
+  return run_sensor(c, c->qbuf[c->cur], d_theta, d_flags, false);
 }
 
 int streams_step(streams_ctx* c, int nsteps) {
@@ -469,17 +476,17 @@ int streams_step(streams_ctx* c, int nsteps) {
   int rc;
   for (int s = 0; s < nsteps; ++s) {
     if (!(c->p.dt_fixed > 0.0)) {
-      k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->wbuf[c->cur], c->partial);
+      k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->partial);
       LAUNCH_CHECK("k_speed_partial");
       k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 1);
       LAUNCH_CHECK("k_dt_final");
     }
     for (int l = 0; l < 3; ++l) {
-      double* w = c->wbuf[c->cur];
+      double* w = c->qbuf[c->cur];
       if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, true))) return rc;
       RhsArgs A;
       std::memset(&A, 0, sizeof A);
-      A.w = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
+      A.q = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
       if (c->p.forcing) {
         // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
         double* Sp = c->S[c->scur];
@@ -492,13 +499,13 @@ int streams_step(streams_ctx* c, int nsteps) {
           LAUNCH_CHECK("k_weno_apply");
         }
         if ((rc = force_from_partials(c, Sc, partial_ok))) return rc;
-        k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1);
+        k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1, l < 2 ? 1 : 0);
         LAUNCH_CHECK("k_update");
         c->scur ^= 1;
       } else {
         // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
-        double* wn = c->wbuf[c->cur ^ 1];
-        A.w_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0];
+        double* wn = c->qbuf[c->cur ^ 1];
+        A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0];
         if ((rc = launch_rhs(c, true, A))) return rc;
         if (c->p.weno_enable) {
           k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->S[0], wn, beta[l]);
@@ -519,7 +526,7 @@ int streams_diagnostics(streams_ctx* c, streams_diag* out) {
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   std::memset(out, 0, sizeof *out);
   const int rg = rgrid_for(c->P.N);
-  const double* w = c->wbuf[c->cur];
+  const double* w = c->qbuf[c->cur];
   int rc;
   // sensor statistics of the current state (interface counts as the next RHS would see them)
   if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, false))) return rc;

@@ -87,7 +87,9 @@ def check_flags(env, o, g, sync=False):
         g.set_state(env[0].from_numpy(o.get_state()).cuda())
     th_o, fl_o = o.sensor()
     th_g, fl_g = g.sensor()
-    assert np.abs(th_g.cpu().numpy() - th_o).max() < 1e-12
+    # theta = -div / sqrt(div^2 + |curl|^2 + eps): a velocity rounding error delta gives |d theta| <= delta/(h sqrt(eps));
+    # with delta ~ 2e-16 |u|, 1/h ~ 2e2 and eps down to 1e-6 (Sod tube) that is ~1e-10; the flags must agree exactly
+    assert np.abs(th_g.cpu().numpy() - th_o).max() < 1e-10
     assert np.array_equal(fl_g.cpu().numpy(), fl_o)
     return int(fl_o.sum())
 
@@ -170,7 +172,11 @@ def test_errors_and_noop(env):
     w0 = torch.from_numpy(wl.state()).cuda()
     g.set_state(w0)
     g.step(0)
-    assert torch.equal(g.get_state(), w0)
+    # the library keeps the state as primitives: get_state(set_state(w)) is w up to the
+    # rounding of one division and one multiplication per component, not bitwise
+    back = g.get_state()
+    for v in range(5):
+        assert float((back[v] - w0[v]).abs().max()) <= 4e-16 * float(w0[v].abs().max())
     assert g.diagnostics().step == 0
     bad = w0.clone()
     bad[0, 0, 0, 0] = -1.0
