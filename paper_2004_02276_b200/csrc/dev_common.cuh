@@ -1,9 +1,10 @@
 // dev_common.cuh -- device-side parameters, ghost-by-index rules (S1) and primitives (S3).
 //
 // State layout in HBM: the library keeps the flow state as PRIMITIVES
-//   Q[6][nz][ny][nx] = rho, u, v, w, T, mu        (x fastest, no ghost nodes stored)
-// so that no kernel pays a division or the power-law viscosity when it loads a stencil point;
-// the conservative vector of PAPER.md:95 is formed in registers where Eq. 11 needs it.
+//   Q[7][nz][ny][nx] = rho, u, v, w, T, mu, H     (x fastest, no ghost nodes stored)
+// so that no kernel pays a division, the power-law viscosity or the total enthalpy when it loads
+// a stencil point (a tile is filled by plain asynchronous copies); the conservative vector of
+// PAPER.md:95 is formed in registers where Eq. 11 needs it.
 // No ghost node is ever stored: a kernel asks `resolve_xy` where the value of an in-plane
 // location (i,j), indices in [-3, n+3), comes from, and `map_z` for the plane (S1;
 // PAPER.md:110, 126, 146).  The composition order x -> y -> z of the ghost rules is reproduced
@@ -15,13 +16,18 @@
 namespace streams {
 
 constexpr int HALO = 3;
-constexpr int NQ = 6;                 // stored primitives per node
+constexpr int NQ = 7;                 // stored primitives per node
 
 enum { BC_PERIODIC = 0, BC_WALL_STAG = 1, BC_WALL_NODE = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_SHOCKGEN = 5, BC_EXTRAP = 6 };
 enum { VISC_POWER = 0, VISC_SUTH = 1 };
 
 // central coefficients of order 2L, zero-padded to three entries
-struct Coef { double a[3], b[3]; };
+struct Coef {
+  double a[3], b[3];
+  double qa[3];      // a_l / 4        (Eq. 6: the 1/4 of the triple average times 2 a_l / 2)
+  double aR[3];      // a_l * Rgas     (pressure difference formed as Rgas * (rho T) differences)
+  double sb2;        // 2 (b_1 + b_2 + b_3)
+};
 
 struct DevP {
   int nx, ny, nz, nxy;
@@ -32,17 +38,17 @@ struct DevP {
   double mu_ref, T_ref, inv_Tref, visc_exp, suth_S;
   double th_thr, th_eps;
   double Twall[2], mu_wall[2];
-  double fs[6], post[6];             // shock generator states as rho,u,v,w,T,mu
+  double fs[NQ], post[NQ];           // shock generator states as rho,u,v,w,T,mu,H
   Coef c;
   // O(n) arrays on the device (owned by the context)
   const double* ih[3];               // 1 / h_d(i)                       (S2)
   const double* gh[3];               // - g_d(i) / h_d(i)^3              (S2)
   const double* hh[3];               // h_d(i)
   const unsigned char* xpost;        // [nx+6]: 1 where the ghost-extended x is behind the generator shock
-  const double* inflow;              // [6][nz][ny] frozen inflow plane (primitives)
+  const double* inflow;              // [NQ][nz][ny] frozen inflow plane (primitives)
 };
 
-struct Prim { double rho, u, v, w, T, mu; };
+struct Prim { double rho, u, v, w, T, mu, H; };
 
 __device__ __forceinline__ int wrap(int i, int n) {
   while (i < 0) i += n;
@@ -71,6 +77,7 @@ __device__ __forceinline__ void cons2prim(const DevP& P, double r, double ru, do
   const double p0 = P.gm1 * (rE - r * ke);
   q.T = p0 * ir * P.inv_R;
   q.mu = visc_mu(P, q.T);
+  q.H = fma(P.cp, q.T, ke);
 }
 __device__ __forceinline__ void prim2cons(const DevP& P, const Prim& q, double wv[5]) {
   wv[0] = q.rho; wv[1] = q.rho * q.u; wv[2] = q.rho * q.v; wv[3] = q.rho * q.w;
@@ -92,10 +99,11 @@ __device__ __forceinline__ void advance_prim(const DevP& P, Prim& q, const doubl
   q.T = fma(dE - dke, P.inv_cv, q.T);
   q.rho = rn; q.u = un; q.v = vn; q.w = wn;
   q.mu = visc_mu(P, q.T);
+  q.H = fma(P.cp, q.T, 0.5 * fma(un, un, fma(vn, vn, wn * wn)));
 }
 // S1: Dirichlet override of a WALL_ISO_NODE wall node after every stage (rho evolves by the scheme)
 __device__ __forceinline__ void wall_node_override(const DevP& P, double Tw, double mu_w, Prim& q) {
-  q.u = 0.0; q.v = 0.0; q.w = 0.0; q.T = Tw; q.mu = mu_w;
+  q.u = 0.0; q.v = 0.0; q.w = 0.0; q.T = Tw; q.mu = mu_w; q.H = P.cp * Tw;
 }
 
 // index maps ----------------------------------------------------------------------------------
@@ -172,22 +180,23 @@ __device__ __forceinline__ void reflect(const DevP& P, double Tw, Prim& q) {
   q.u = -q.u; q.v = -q.v; q.w = -q.w;
   q.T = Tg;
   q.mu = visc_mu_outofline(Tg, P.mu_ref, P.T_ref, P.inv_Tref, P.visc_exp, P.suth_S, P.visc_model);
+  q.H = fma(P.cp, Tg, 0.5 * fma(q.u, q.u, fma(q.v, q.v, q.w * q.w)));
 }
 
-// raw load of the six primitives for source s in (already mapped) plane kk; reflection NOT applied
+// raw load of the stored primitives for source s in (already mapped) plane kk; reflection NOT applied
 __device__ __forceinline__ void load_src_raw(const DevP& P, const double* __restrict__ Q, const Src s, int kk, Prim& q) {
   const int k = s.kind & 7;
   if (k == SRC_FIELD) {
     const size_t o = (size_t)kk * P.nxy + s.off;
     q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.N); q.v = __ldg(Q + o + 2 * P.N); q.w = __ldg(Q + o + 3 * P.N);
-    q.T = __ldg(Q + o + 4 * P.N); q.mu = __ldg(Q + o + 5 * P.N);
+    q.T = __ldg(Q + o + 4 * P.N); q.mu = __ldg(Q + o + 5 * P.N); q.H = __ldg(Q + o + 6 * P.N);
   } else if (k == SRC_INFLOW) {
     const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
     q.rho = P.inflow[o]; q.u = P.inflow[o + st]; q.v = P.inflow[o + 2 * st]; q.w = P.inflow[o + 3 * st];
-    q.T = P.inflow[o + 4 * st]; q.mu = P.inflow[o + 5 * st];
+    q.T = P.inflow[o + 4 * st]; q.mu = P.inflow[o + 5 * st]; q.H = P.inflow[o + 6 * st];
   } else {
     const double* c = k == SRC_POST ? P.post : P.fs;
-    q.rho = c[0]; q.u = c[1]; q.v = c[2]; q.w = c[3]; q.T = c[4]; q.mu = c[5];
+    q.rho = c[0]; q.u = c[1]; q.v = c[2]; q.w = c[3]; q.T = c[4]; q.mu = c[5]; q.H = c[6];
   }
 }
 __device__ __forceinline__ void apply_reflect(const DevP& P, const Src s, Prim& q) {

@@ -18,12 +18,12 @@ struct DevScal {
   unsigned int pad;
 };
 
-// ---- S3: conservative w[5][N] -> primitives Q[6][N]  (streams_set_state) ----
+// ---- S3: conservative w[5][N] -> primitives Q[NQ][N]  (streams_set_state) ----
 __global__ void __launch_bounds__(RT) k_cons2prim(const DevP P, const double* __restrict__ w, double* __restrict__ Q) {
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     Prim q;
     cons2prim(P, w[o], w[o + P.N], w[o + 2 * P.N], w[o + 3 * P.N], w[o + 4 * P.N], q);
-    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu;
+    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu; Q[o + 6 * P.N] = q.H;
   }
 }
 // ---- primitives -> conservative (streams_get_state) ----
@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(RT) k_update(const DevP P, double* __restrict_
     const int j = (int)((o / P.nx) % P.ny);
     if (j == 0 && P.bc[2] == BC_WALL_NODE) wall_node_override(P, P.Twall[0], P.mu_wall[0], q);
     if (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE) wall_node_override(P, P.Twall[1], P.mu_wall[1], q);
-    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu;
+    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu; Q[o + 6 * P.N] = q.H;
   }
 }
 

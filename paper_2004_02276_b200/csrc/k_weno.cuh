@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(128) k_weno_apply(const DevP P, const double* 
 #pragma unroll
         for (int v = 0; v < 5; ++v) dW[v] = dtb * dR[v];
         advance_prim(P, q, dW);
-        q_new[o] = q.rho; q_new[o + P.N] = q.u; q_new[o + 2 * P.N] = q.v; q_new[o + 3 * P.N] = q.w; q_new[o + 4 * P.N] = q.T; q_new[o + 5 * P.N] = q.mu;
+        q_new[o] = q.rho; q_new[o + P.N] = q.u; q_new[o + 2 * P.N] = q.v; q_new[o + 3 * P.N] = q.w; q_new[o + 4 * P.N] = q.T; q_new[o + 5 * P.N] = q.mu; q_new[o + 6 * P.N] = q.H;
       }
     }
   }

@@ -32,7 +32,7 @@ struct streams_ctx {
   DevP P;
   cudaStream_t st;
   // workspace carve-up (caller memory)
-  double *qbuf[2], *S[2], *theta, *partial, *inflow, *speeds;   // qbuf: primitives [6][N]; S: R registers [5][N]
+  double *qbuf[2], *S[2], *theta, *partial, *inflow, *speeds;   // qbuf: primitives [NQ][N]; S: R registers [5][N]
   unsigned char *nflag, *lmask;
   unsigned int* list;
   int npartial;
@@ -75,7 +75,8 @@ int cuda_fail(streams_ctx* c, cudaError_t e, const char* where) {
   } while (0)
 
 bool coeffs(int order, Coef& k) {
-  for (int i = 0; i < 3; ++i) k.a[i] = k.b[i] = 0.0;
+  for (int i = 0; i < 3; ++i) k.a[i] = k.b[i] = k.qa[i] = k.aR[i] = 0.0;
+  k.sb2 = 0.0;
   if (order == 2) { k.a[0] = 0.5; k.b[0] = 1.0; return true; }
   if (order == 4) { k.a[0] = 2.0 / 3.0; k.a[1] = -1.0 / 12.0; k.b[0] = 4.0 / 3.0; k.b[1] = -1.0 / 12.0; return true; }
   if (order == 6) { k.a[0] = 0.75; k.a[1] = -0.15; k.a[2] = 1.0 / 60.0; k.b[0] = 1.5; k.b[1] = -0.15; k.b[2] = 1.0 / 90.0; return true; }
@@ -116,7 +117,7 @@ double visc_host(const streams_params& p, double T) {
 }
 
 // S1 shock generator: weak oblique-shock solution for the deflection angle
-bool shock_post_state(const streams_params& p, double post[6]) {
+bool shock_post_state(const streams_params& p, double post[NQ]) {
   const double g = p.gamma, u1 = p.fs[1], T1 = p.fs[4];
   const double M = u1 / std::sqrt(g * p.Rgas * T1);
   const double tphi = std::tan(p.shock_angle_deg * 3.14159265358979323846 / 180.0);
@@ -145,6 +146,7 @@ bool shock_post_state(const streams_params& p, double post[6]) {
   post[3] = p.fs[3];
   post[4] = T1 * pr / rr;
   post[5] = visc_host(p, post[4]);
+  post[6] = p.gamma * p.Rgas / (p.gamma - 1.0) * post[4] + 0.5 * (post[1] * post[1] + post[2] * post[2] + post[3] * post[3]);
   return true;
 }
 
@@ -312,10 +314,13 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   P.th_thr = p->sensor_threshold; P.th_eps = p->sensor_eps;
   P.Twall[0] = p->T_wall[0]; P.Twall[1] = p->T_wall[1];
   P.mu_wall[0] = visc_host(*p, p->T_wall[0]); P.mu_wall[1] = visc_host(*p, p->T_wall[1]);
+  for (int i = 0; i < 3; ++i) { K.qa[i] = 0.25 * K.a[i]; K.aR[i] = K.a[i] * p->Rgas; }
+  K.sb2 = 2.0 * (K.b[0] + K.b[1] + K.b[2]);
   P.c = K;
   for (int i = 0; i < 5; ++i) P.fs[i] = p->fs[i];
   P.fs[5] = visc_host(*p, p->fs[4]);
-  for (int i = 0; i < 6; ++i) P.post[i] = P.fs[i];
+  P.fs[6] = P.cp * p->fs[4] + 0.5 * (p->fs[1] * p->fs[1] + p->fs[2] * p->fs[2] + p->fs[3] * p->fs[3]);
+  for (int i = 0; i < NQ; ++i) P.post[i] = P.fs[i];
   std::vector<unsigned char> xpost(n[0] + 2 * HALO, 0);
   if (p->bc[3] == STREAMS_BC_SHOCKGEN) {
     if (!shock_post_state(*p, P.post)) { delete c; return fail(nullptr, STREAMS_EINVAL, "shock generator: no attached weak shock for these parameters"); }
@@ -417,8 +422,8 @@ static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A) {
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
-  if (fused) k_rhs<true><<<c->rhs_grid, dim3(TX, TY), smem, c->st>>>(c->P, A);
-  else k_rhs<false><<<c->rhs_grid, dim3(TX, TY), smem, c->st>>>(c->P, A);
+  if (fused) k_rhs<true><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A);
+  else k_rhs<false><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A);
   LAUNCH_CHECK("k_rhs");
   if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
