@@ -58,7 +58,7 @@ def test_workspace_and_validation(blib):
     wl = W.config3_channel(256, 128, 128)
     n = wl.npoints
     nb = blib.workspace_bytes(wl.grid, wl.params)
-    assert (2 * 6 + 2 * 5) * 8 * n <= nb < (2 * 6 + 2 * 5) * 8 * n + (64 << 20)   # two primitive states (6 fields) + two RK registers (5) + small arrays
+    assert (2 * 7 + 2 * 5) * 8 * n <= nb < (2 * 7 + 2 * 5) * 8 * n + (64 << 20)   # two primitive states (7 fields) + two RK registers (5) + small arrays
     wl5 = W.config5_channel_big()
     assert blib.workspace_bytes(wl5.grid, wl5.params) < 60e9          # fits 180 GB HBM with room for the input copy
     bad = dict(wl.params, order=5)
