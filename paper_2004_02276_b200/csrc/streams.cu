@@ -45,6 +45,8 @@ struct streams_ctx {
   long long launches;
   dim3 rhs_grid;
   int lz;
+  CUtensorMap tmap[2];           // TMA descriptors of qbuf[0], qbuf[1] as 4-D tensors (x, y, z, field)
+  int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
   int prof_on, prof_n;
   std::vector<cudaEvent_t>* prof_ev;   // pairs (start, stop) around k_rhs
   char err[256];
@@ -148,6 +150,27 @@ bool shock_post_state(const streams_params& p, double post[NQ]) {
   post[5] = visc_host(p, post[4]);
   post[6] = p.gamma * p.Rgas / (p.gamma - 1.0) * post[4] + 0.5 * (post[1] * post[1] + post[2] * post[2] + post[3] * post[3]);
   return true;
+}
+
+// TMA descriptor of one primitive-state buffer: tensor (x, y, z, field), box = one tile plane with its halo.
+// cuTensorMapEncodeTiled is fetched through the runtime (no link-time dependency on libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool make_tile_map(CUtensorMap* tm, double* q, int nx, int ny, int nz) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess)
+    return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)NQ};
+  const cuuint64_t strides[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)nx * ny * nz * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)PITCH, (cuuint32_t)PY, 1u, (cuuint32_t)NQ};
+  const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+  const CUresult r = ((EncodeTiledFn)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, q, dims, strides, box, estr,
+                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
 }
 
 struct Carve { size_t off = 0; size_t take(size_t bytes) { size_t o = off; off += up(bytes); return o; } };
@@ -353,6 +376,14 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   e = cudaStreamSynchronize(c->st);     // host vectors go out of scope
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "create sync"); }
 
+  // TMA needs 16-byte global strides: rows of an even number of doubles.  Odd nx takes the by-index fill.
+  c->use_tma = (n[0] % 2 == 0) ? 1 : 0;
+  if (c->use_tma)
+    for (int i = 0; i < 2; ++i)
+      if (!make_tile_map(&c->tmap[i], c->qbuf[i], n[0], n[1], n[2])) {
+        cudaFree(c->small_dev); delete c;
+        return fail(nullptr, STREAMS_ECUDA, "cuTensorMapEncodeTiled failed");
+      }
   e = cudaFuncSetAttribute(k_rhs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaFuncSetAttribute(k_rhs)"); }
@@ -418,12 +449,15 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
   return STREAMS_OK;
 }
 
-static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A) {
+static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A_in) {
+  RhsArgs A = A_in;
+  A.use_tma = c->use_tma;
+  const CUtensorMap& tm = c->tmap[A.q == c->qbuf[1] ? 1 : 0];
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
-  if (fused) k_rhs<true><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A);
-  else k_rhs<false><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A);
+  if (fused) k_rhs<true><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);
+  else k_rhs<false><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);
   LAUNCH_CHECK("k_rhs");
   if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
