@@ -19,7 +19,7 @@ struct DevScal {
 };
 
 // ---- S3: conservative w[5][N] -> primitives Q[NQ][N]  (streams_set_state) ----
-__global__ void __launch_bounds__(RT) k_cons2prim(const DevP P, const double* __restrict__ w, double* __restrict__ Q) {
+__global__ void __launch_bounds__(RT) k_cons2prim(const __grid_constant__ DevP P, const double* __restrict__ w, double* __restrict__ Q) {
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     Prim q;
     cons2prim(P, w[o], w[o + P.N], w[o + 2 * P.N], w[o + 3 * P.N], w[o + 4 * P.N], q);
@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(RT) k_cons2prim(const DevP P, const double* __
   }
 }
 // ---- primitives -> conservative (streams_get_state) ----
-__global__ void __launch_bounds__(RT) k_prim2cons(const DevP P, const double* __restrict__ Q, double* __restrict__ w) {
+__global__ void __launch_bounds__(RT) k_prim2cons(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ w) {
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     Prim q;
     q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(RT) k_prim2cons(const DevP P, const double* __
 
 // ---- S11 with S9: R += f (0,1,0,0,u);  w <- w + dt (alpha R_prev + beta R), Eq. 11, state kept
 // as primitives.  `keep_R` != 0 writes the two forced components of R back (the next stage reads them as R_prev).
-__global__ void __launch_bounds__(RT) k_update(const DevP P, double* __restrict__ Q, const double* __restrict__ Sp,
+__global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, double* __restrict__ Q, const double* __restrict__ Sp,
                                                double* __restrict__ Sc, const DevScal* __restrict__ sc,
                                                double alpha, double beta, int use_force, int keep_R) {
   const double dt = sc->dt;
@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(RT) k_update(const DevP P, double* __restrict_
 }
 
 // R_rhou += f, R_rhoE += f u  (streams_rhs with forcing)
-__global__ void __launch_bounds__(RT) k_apply_force(const DevP P, const double* __restrict__ Q, double* __restrict__ R,
+__global__ void __launch_bounds__(RT) k_apply_force(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ R,
                                                     const DevScal* __restrict__ sc) {
   const double f = sc->force;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(RT) k_apply_force(const DevP P, const double* 
 }
 
 // ---- S9: per-block partial sums of R_rhou * vol ----
-__global__ void __launch_bounds__(RT) k_force_partial(const DevP P, const double* __restrict__ R, double* __restrict__ partial) {
+__global__ void __launch_bounds__(RT) k_force_partial(const __grid_constant__ DevP P, const double* __restrict__ R, double* __restrict__ partial) {
   __shared__ double sh[RT / 32];
   double acc = 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(RT) k_force_final(const double* __restrict__ p
 }
 
 // ---- S10: dt = cfl / max_d max_nodes (|u_d| + c) / h_d ----
-__global__ void __launch_bounds__(RT) k_speed_partial(const DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[3][grid]*/) {
+__global__ void __launch_bounds__(RT) k_speed_partial(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[3][grid]*/) {
   __shared__ double sh[RT / 32];
   double m[3] = {0.0, 0.0, 0.0};
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
@@ -131,7 +131,7 @@ __global__ void k_advance_time(DevScal* sc) { sc->time += sc->dt; }
 
 // ---- diagnostics: per-block partials, reduced on the host by streams_diagnostics ----
 constexpr int NDIAG = 12;   // mass, mx, my, mz, E, ke, vol | min rho, min p, max Mach | nonfinite | spare
-__global__ void __launch_bounds__(RT) k_diag_partial(const DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[NDIAG][grid]*/) {
+__global__ void __launch_bounds__(RT) k_diag_partial(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[NDIAG][grid]*/) {
   __shared__ double sh[RT / 32];
   double s[7] = {0, 0, 0, 0, 0, 0, 0};
   double mnr = INFINITY, mnp = INFINITY, mxm = 0.0, bad = 0.0;
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(RT) k_diag_partial(const DevP P, const double*
 }
 
 // capture the frozen inflow plane (S1 INFLOW_FROZEN): inflow[v][k][j] = Q[v][k][j][0]
-__global__ void k_capture_inflow(const DevP P, const double* __restrict__ Q, double* __restrict__ inflow) {
+__global__ void k_capture_inflow(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ inflow) {
   const long long n = (long long)P.nz * P.ny;
   for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < NQ * n; e += (long long)gridDim.x * blockDim.x) {
     const int v = (int)(e / n);

@@ -47,8 +47,11 @@ constexpr int SM_STGX = PY * TX;                // D_x u on the y-extended colum
 constexpr int SM_STG1 = SM_STGY + SM_STGX;      // one staging set; two sets alternate between planes
 constexpr int SM_GRING = 7 * 3 * NPT;
 constexpr int SM_RRING = 4 * 5 * NPT;
+constexpr int NOWN = 2;                         // own-node ring: plane s+4 is read while s+5 is in flight
+constexpr int SM_OWN = NOWN * NF * NPT;
 constexpr int SM_RED = 32;
-constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_RED + 4;
+constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_RED + 4;
+static_assert(SM_RHS_DOUBLES * 8 <= 227 * 1024, "one CTA per SM: the shared-memory budget of sm_100a");
 constexpr int NSTAGE = 2 * HALO * TY + 2 * HALO * TX;                     // 240 staged derivatives outside the tile
 constexpr unsigned TILE_BYTES = SM_TILE1 * sizeof(double);
 static_assert(TILE_BYTES % 128 == 0, "TMA destination buffers stay 128-byte aligned");
@@ -86,6 +89,13 @@ __device__ __forceinline__ void tma_tile(unsigned dst, const CUtensorMap* tm, in
   asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                ::"r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(0), "r"(bar) : "memory");
 }
+// thread-private asynchronous 8-byte copies (own node of a later plane into the own-node ring)
+__device__ __forceinline__ void cp_async8(unsigned dst, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 struct Nb { double rho, u, v, w, T, mu, H; };
@@ -244,7 +254,10 @@ __device__ __forceinline__ void visc_assemble(const DevP& P, const Nb& c, NodeAc
 
 // S8: characteristic form of the x-derivative at the outflow node, incoming waves removed.
 // Replaces the index-space flux difference f of the x direction.  Rare path (one column): kept out of line.
-__device__ __noinline__ void outflow_x(const DevP& P, const double* __restrict__ t, int oc, double* __restrict__ f) {
+struct F5 { double v[5]; };   // returned by value: stays in registers across the call (no local-memory frame)
+__device__ __noinline__ F5 outflow_x(const DevP& P, const double* __restrict__ t, int oc) {
+  F5 r;
+  double* f = r.v;
   const Nb c = tile_nb(t, oc), n1 = tile_nb(t, oc - 1), n2 = tile_nb(t, oc - 2);
   const double pc = c.rho * (P.Rgas * c.T), p1 = n1.rho * (P.Rgas * n1.T), p2 = n2.rho * (P.Rgas * n2.T);
   const double w0[5] = {c.rho, c.rho * c.u, c.rho * c.v, c.rho * c.w, c.rho * c.H - pc};
@@ -273,25 +286,29 @@ __device__ __noinline__ void outflow_x(const DevP& P, const double* __restrict__
   f[2] = v_ * Ls[0] + v_ * Ls[1] + Ls[2] + v_ * Ls[4];
   f[3] = w_ * Ls[0] + w_ * Ls[1] + Ls[3] + w_ * Ls[4];
   f[4] = (Hc - u * cs) * Ls[0] + 0.5 * q2 * Ls[1] + v_ * Ls[2] + w_ * Ls[3] + (Hc + u * cs) * Ls[4];
+  return r;
 }
 
 // flux difference of the y direction next to a staggered wall: the wall-plane flux keeps the pressure only
-__device__ __noinline__ void wall_y(const DevP& P, const double* __restrict__ t, int oc, bool wall_lo, bool wall_hi, double* __restrict__ f) {
+__device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, int oc, bool wall_lo, bool wall_hi) {
+  F5 r;
   double Fp[5] = {0, 0, 0, 0, 0}, Fm[5] = {0, 0, 0, 0, 0};
   if (wall_hi) Fp[2] = flux_y_pressure(P, t, oc, PITCH); else flux_y_full(P, t, oc, PITCH, Fp);
   if (wall_lo) Fm[2] = flux_y_pressure(P, t, oc - PITCH, PITCH); else flux_y_full(P, t, oc - PITCH, PITCH, Fm);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) f[v] = Fp[v] - Fm[v];
+  for (int v = 0; v < 5; ++v) r.v[v] = Fp[v] - Fm[v];
+  return r;
 }
 
 template <bool FUSED>
-__global__ void __launch_bounds__(NT, 1) k_rhs(const DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
+__global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) double sm[];
   double* tiles = sm;
   double* stg = tiles + SM_TILES;
   double* gring = stg + 2 * SM_STG1;
   double* rring = gring + SM_GRING;
-  double* red = rring + SM_RRING;
+  double* oring = rring + SM_RRING;
+  double* red = oring + SM_OWN;
   const unsigned bar0 = smem_u32(red + SM_RED);          // NBUF mbarriers: tile buffer b holds its plane
 
   const int tid = threadIdx.x;
@@ -350,6 +367,15 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const DevP P, const RhsArgs A, co
       Tw[a] = __ldg(q + 4 * P.N); mw[a] = __ldg(q + 5 * P.N); Hw[a] = __ldg(q + 6 * P.N);
     }
   }
+  // own node of the planes ahead: plane s+5 is requested at the top of step s (cp.async, thread-private
+  // slot, no register and no barrier), plane s+4 is taken from the ring at the end of step s
+  const unsigned own0 = smem_u32(oring + tid);
+  if (active) {
+    const double* q = qown + (size_t)map_z(P, k0 + 1) * P.nxy;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) cp_async8(own0 + ((1 * NF + f) * NPT) * 8, q + f * P.N);
+  }
+  cp_async_commit();
   const double dt = FUSED ? *A.dt_ptr : 0.0;
   int slot7 = 0, buf = 0;                                // it % 7, it % NBUF
   unsigned phase = 0;                                    // (it / NBUF) & 1
@@ -357,6 +383,13 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const DevP P, const RhsArgs A, co
   for (int s = k0 - 3, it = 0; s < k1 + 3; ++s, ++it) {
     const bool full = s >= k0 && s < k1;
     double* t = tiles + buf * SM_TILE1;
+    if (active && s + 5 < k1 + 3) {
+      const double* q = qown + (size_t)map_z(P, s + 5) * P.nxy;
+      const unsigned d = own0 + ((it & 1) * NF * NPT) * 8;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.N);
+    }
+    cp_async_commit();
     if (use_tma) mbar_wait(bar0 + 8 * buf, phase);
     if (edge) {
       fill_by_index(P, A.q, i0, j0, map_z(P, s), t, !use_tma, tid);
@@ -418,7 +451,11 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const DevP P, const RhsArgs A, co
           }
           double f[5];
           conv_from_acc<0>(c, X, f);
-          if (gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) outflow_x(P, t, oc, f);
+          if (gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) {
+            const F5 r = outflow_x(P, t, oc);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) f[v] = r.v[v];
+          }
           dir_fold<0>(P, c, X, f, ihx, ghx, N);
         }
         // ---- y ----
@@ -434,7 +471,11 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const DevP P, const RhsArgs A, co
           conv_from_acc<1>(c, Y, f);
           const bool wall_lo = gj == 0 && P.bc[2] == BC_WALL_STAG;
           const bool wall_hi = gj == P.ny - 1 && P.bc[3] == BC_WALL_STAG;
-          if (wall_lo || wall_hi) wall_y(P, t, oc, wall_lo, wall_hi, f);
+          if (wall_lo || wall_hi) {
+            const F5 r = wall_y(P, t, oc, wall_lo, wall_hi);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) f[v] = r.v[v];
+          }
           dir_fold<1>(P, c, Y, f, ihy, ghy, N);
         }
         g1 = N.G[6]; g2 = N.G[7]; g3 = N.G[0] + N.G[4];
@@ -515,10 +556,11 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const DevP P, const RhsArgs A, co
     for (int a = 0; a < 6; ++a) {
       rw[a] = rw[a + 1]; uw[a] = uw[a + 1]; vw[a] = vw[a + 1]; ww[a] = ww[a + 1]; Tw[a] = Tw[a + 1]; mw[a] = mw[a + 1]; Hw[a] = Hw[a + 1];
     }
+    cp_async_wait<1>();                                  // plane s+4 has landed (requested at step s-1)
     if (active && s + 4 < k1 + 3) {
-      const double* q = qown + (size_t)map_z(P, s + 4) * P.nxy;
-      rw[6] = __ldg(q); uw[6] = __ldg(q + P.N); vw[6] = __ldg(q + 2 * P.N); ww[6] = __ldg(q + 3 * P.N);
-      Tw[6] = __ldg(q + 4 * P.N); mw[6] = __ldg(q + 5 * P.N); Hw[6] = __ldg(q + 6 * P.N);
+      const double* o = oring + ((it + 1) & 1) * NF * NPT + tid;
+      rw[6] = o[F_RHO * NPT]; uw[6] = o[F_U * NPT]; vw[6] = o[F_V * NPT]; ww[6] = o[F_W * NPT];
+      Tw[6] = o[F_T * NPT]; mw[6] = o[F_MU * NPT]; Hw[6] = o[F_H * NPT];
     }
   }
   if (A.partial) {

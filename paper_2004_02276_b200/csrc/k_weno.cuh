@@ -14,7 +14,7 @@
 namespace streams {
 
 // ---- S4: theta of Eq. 8 per node -> byte flag theta > theta_th ----
-__global__ void __launch_bounds__(RT) k_sensor(const DevP P, const double* __restrict__ w, unsigned char* __restrict__ nflag,
+__global__ void __launch_bounds__(RT) k_sensor(const __grid_constant__ DevP P, const double* __restrict__ w, unsigned char* __restrict__ nflag,
                                                double* __restrict__ theta_out, DevScal* sc) {
   __shared__ double sh[RT / 32];
   double tmax = 0.0;
@@ -66,7 +66,7 @@ __device__ __forceinline__ int iface_flag(const DevP& P, const unsigned char* __
 }
 
 // list of nodes with a flagged interface; entry = node index, mask bit (2d+side), side 0 = below, 1 = above
-__global__ void __launch_bounds__(RT) k_weno_list(const DevP P, const unsigned char* __restrict__ nflag,
+__global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P, const unsigned char* __restrict__ nflag,
                                                   unsigned int* __restrict__ list, unsigned char* __restrict__ lmask,
                                                   unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
   unsigned long long cnt[3] = {0, 0, 0};
@@ -203,7 +203,7 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
 
 // one thread per listed node: R += dR, and (if q_new) the node of the already advanced state takes the
 // conservative increment dt beta dR  (Eq. 11 is linear in R)
-__global__ void __launch_bounds__(128) k_weno_apply(const DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
+__global__ void __launch_bounds__(128) k_weno_apply(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
                                                     const unsigned char* __restrict__ lmask, const DevScal* __restrict__ sc,
                                                     double* __restrict__ R, double* __restrict__ q_new, double beta) {
   const unsigned int n = sc->list_count;
