@@ -46,11 +46,14 @@ constexpr int SM_STGY = TY * PITCH;             // D_y v on the x-extended rows
 constexpr int SM_STGX = PY * TX;                // D_x u on the y-extended columns
 constexpr int SM_STG1 = SM_STGY + SM_STGX;      // one staging set; two sets alternate between planes
 constexpr int SM_GRING = 7 * 3 * NPT;
-constexpr int SM_RRING = 4 * 5 * NPT;
-constexpr int NOWN = 2;                         // own-node ring: plane s+4 is read while s+5 is in flight
+constexpr int SM_RRING = 3 * 5 * NPT;     // R of planes s-1..s-3: read (plane s-3) before written (plane s) in a step
+constexpr int NOWN = 3;                         // own-node ring: plane s+3 is read while s+4, s+5 are in flight
 constexpr int SM_OWN = NOWN * NF * NPT;
 constexpr int SM_RED = 32;
-constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_RED + 4;
+constexpr int LZ_MAX = 128;                     // planes per CTA (make_layout caps the chunk length)
+constexpr int SM_MET = 3 * LZ_MAX + 2 * TX + 2 * TY;   // 1/h_z, -g_z/h_z^3, h_z of the chunk; 1/h, -g/h^3 of the tile's x and y
+constexpr int SM_PATCH = TILE;                  // ghost-slot list of an edge tile: one int2 (8 bytes) per entry
+constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_MET + SM_PATCH + SM_RED + 8;
 static_assert(SM_RHS_DOUBLES * 8 <= 227 * 1024, "one CTA per SM: the shared-memory budget of sm_100a");
 constexpr int NSTAGE = 2 * HALO * TY + 2 * HALO * TX;                     // 240 staged derivatives outside the tile
 constexpr unsigned TILE_BYTES = SM_TILE1 * sizeof(double);
@@ -76,6 +79,9 @@ __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
   unsigned ok;
@@ -193,20 +199,30 @@ __device__ __forceinline__ double d1_tile(const DevP& P, const double* __restric
   return d1;
 }
 
-// ---- S1 by index: patch the ghost slots of an edge tile (all = false) or fill every slot (all = true, no TMA) ----
-__device__ __noinline__ void fill_by_index(const DevP& P, const double* __restrict__ Q, int i0, int j0, int kk,
-                                           double* __restrict__ t, bool all, int tid) {
+// ---- S1 by index: the ghost slots of an edge tile (all = false) or every slot (all = true, no TMA) ----
+// The list is built once per CTA; entry = (tile slot | kind << 16, in-plane source offset).
+__device__ __noinline__ void build_patch_list(const DevP& P, int i0, int j0, bool all, int2* __restrict__ list, int* __restrict__ count, int tid) {
   for (int e = tid; e < TILE; e += NT) {
     const int r = e / PITCH, io = e - r * PITCH - XH, jo = r - HALO;
     if (io < -HALO || io >= TX + HALO) continue;
     const int gi = i0 + io, gj = j0 + jo;
     if (gi >= P.nx + HALO || gj >= P.ny + HALO) continue;
-    if (!all && gi >= 0 && gi < P.nx && gj >= 0 && gj < P.ny) continue;      // TMA brought it
+    if (!all && gi >= 0 && gi < P.nx && gj >= 0 && gj < P.ny) continue;      // TMA brings it
     const Src s = resolve_xy(P, gi, gj);
+    const int n = atomicAdd(count, 1);
+    list[n] = make_int2(e | (s.kind << 16), s.off);
+  }
+}
+// fill the listed slots of tile `t` for (already mapped) plane kk
+__device__ __noinline__ void patch_tile(const DevP& P, const double* __restrict__ Q, const int2* __restrict__ list, int n, int kk,
+                                        double* __restrict__ t, int tid) {
+  for (int e = tid; e < n; e += NT) {
+    const int2 en = list[e];
+    Src s; s.kind = en.x >> 16; s.off = en.y;
     Prim q;
     load_src_raw(P, Q, s, kk, q);
     apply_reflect(P, s, q);
-    double* d = t + e;
+    double* d = t + (en.x & 0xffff);
     d[F_RHO * TILE] = q.rho; d[F_U * TILE] = q.u; d[F_V * TILE] = q.v; d[F_W * TILE] = q.w;
     d[F_T * TILE] = q.T; d[F_MU * TILE] = q.mu; d[F_H * TILE] = q.H;
   }
@@ -300,6 +316,7 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
   return r;
 }
 
+
 template <bool FUSED>
 __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) double sm[];
@@ -308,8 +325,19 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   double* gring = stg + 2 * SM_STG1;
   double* rring = gring + SM_GRING;
   double* oring = rring + SM_RRING;
-  double* red = oring + SM_OWN;
+  double* met = oring + SM_OWN;
+  int2* plist = reinterpret_cast<int2*>(met + SM_MET);
+  double* red = met + SM_MET + SM_PATCH;
   const unsigned bar0 = smem_u32(red + SM_RED);          // NBUF mbarriers: tile buffer b holds its plane
+  const unsigned sbar = bar0 + 8 * NBUF;                 // the per-plane CTA barrier, split into arrive / wait
+  int* pcount = reinterpret_cast<int*>(red + SM_RED + NBUF + 1);
+  const double* zi = met;                                // 1/h_z, -g_z/h_z^3, h_z of planes k0 .. k1-1
+  const double* zg = met + LZ_MAX;
+  const double* zh = met + 2 * LZ_MAX;
+  const double* xi = met + 3 * LZ_MAX;                   // 1/h_x, -g_x/h_x^3 of the tile's columns
+  const double* xg = xi + TX;
+  const double* yi = xg + TX;                            // 1/h_y, -g_y/h_y^3 of the tile's rows
+  const double* yg = yi + TY;
 
   const int tid = threadIdx.x;
   const int ti = tid & (TX - 1), tj = tid / TX;
@@ -321,61 +349,90 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const int oc = (tj + HALO) * PITCH + ti + XH;                               // own tile offset
   const int own_off = gj * P.nx + gi;
   const bool use_tma = A.use_tma != 0;
-  // tiles that see a domain face patch their ghost slots by index (S1); without TMA every tile fills every slot
+  // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
   const bool edge = !use_tma || i0 < HALO || i0 + TX + HALO > P.nx || j0 < HALO || j0 + TY + HALO > P.ny;
   const int nplanes = k1 + 3 - (k0 - 3);
 
-  if (use_tma && tid == 0) {
+  if (tid == 0) {
+    *pcount = 0;
+    mbar_init(sbar, NT / 32);
+    if (use_tma) {
 #pragma unroll
-    for (int b = 0; b < NBUF; ++b) mbar_init(bar0 + 8 * b, 1);
+      for (int b = 0; b < NBUF; ++b) mbar_init(bar0 + 8 * b, 1);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
+    if (use_tma) {
 #pragma unroll
-    for (int b = 0; b < 2; ++b)
-      if (b < nplanes) {
-        mbar_expect_tx(bar0 + 8 * b, TILE_BYTES);
-        tma_tile(smem_u32(tiles + b * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, k0 - 3 + b), bar0 + 8 * b);
-      }
+      for (int b = 0; b < 2; ++b)
+        if (b < nplanes) {
+          mbar_expect_tx(bar0 + 8 * b, TILE_BYTES);
+          tma_tile(smem_u32(tiles + b * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, k0 - 3 + b), bar0 + 8 * b);
+        }
+    }
+  }
+  for (int e = tid; e < k1 - k0; e += NT) {
+    met[e] = P.ih[2][k0 + e]; met[LZ_MAX + e] = P.gh[2][k0 + e]; met[2 * LZ_MAX + e] = P.hh[2][k0 + e];
+  }
+  if (tid < TX) {
+    const bool ok = i0 + tid < P.nx;
+    met[3 * LZ_MAX + tid] = ok ? P.ih[0][i0 + tid] : 0.0;
+    met[3 * LZ_MAX + TX + tid] = ok ? P.gh[0][i0 + tid] : 0.0;
+  } else if (tid < TX + TY) {
+    const int r = tid - TX;
+    const bool ok = j0 + r < P.ny;
+    met[3 * LZ_MAX + 2 * TX + r] = ok ? P.ih[1][j0 + r] : 0.0;
+    met[3 * LZ_MAX + 2 * TX + TY + r] = ok ? P.gh[1][j0 + r] : 0.0;
   }
   __syncthreads();
+  int npatch = 0;
+  if (edge) {
+    build_patch_list(P, i0, j0, !use_tma, plist, pcount, tid);
+    __syncthreads();
+    npatch = *pcount;
+    if (use_tma) mbar_wait(bar0, 0);
+    patch_tile(P, A.q, plist, npatch, map_z(P, k0 - 3), tiles, tid);     // first plane; later planes one step ahead
+    __syncthreads();
+  }
 
-  const double ihx = active ? P.ih[0][gi] : 0.0, ihy = active ? P.ih[1][gj] : 0.0;
-  const double ghx = active ? P.gh[0][gi] : 0.0, ghy = active ? P.gh[1][gj] : 0.0;
-  const double hxy = active ? P.hh[0][gi] * P.hh[1][gj] : 0.0;
   double fsum = 0.0;
 
   // staged derivative outside the tile: [0,48) D_y v on the x-halo columns, [48,240) D_x u on the y-halo rows
-  int sj_src = 0, sj_dst = -1, sj_st = 1, sj_f = F_U;
+  int sj_src = 0, sj_dst = -1, sj_st = 1;
   if (tid < 2 * HALO * TY) {
     const int r = tid / 6, c = tid % 6, io = c < 3 ? c - 3 : TX + c - 3;
-    sj_src = (r + HALO) * PITCH + io + XH; sj_dst = r * PITCH + io + XH; sj_st = PITCH; sj_f = F_V;
+    sj_src = F_V * TILE + (r + HALO) * PITCH + io + XH; sj_dst = r * PITCH + io + XH; sj_st = PITCH;
   } else if (tid < NSTAGE) {
     const int e2 = tid - 2 * HALO * TY, rr = e2 / TX, col = e2 % TX, jo = rr < 3 ? rr - 3 : TY + rr - 3;
-    sj_src = (jo + HALO) * PITCH + col + XH; sj_dst = SM_STGY + (jo + HALO) * TX + col; sj_st = 1; sj_f = F_U;
+    sj_src = F_U * TILE + (jo + HALO) * PITCH + col + XH; sj_dst = SM_STGY + (jo + HALO) * TX + col; sj_st = 1;
   }
 
   // register windows of the own node: index a holds plane s-3+a
   const double* qown = A.q + own_off;
-  double rw[7], uw[7], vw[7], ww[7], Tw[7], mw[7], Hw[7];
+  // (plane s+3 stays in the own-node ring: read for the l = 3 pair and again when it enters the window)
+  double rw[6], uw[6], vw[6], ww[6], Tw[6], mw[6], Hw[6];
 #pragma unroll
-  for (int a = 0; a < 7; ++a) { rw[a] = 1.0; uw[a] = vw[a] = ww[a] = 0.0; Tw[a] = mw[a] = 1.0; Hw[a] = 0.0; }
+  for (int a = 0; a < 6; ++a) { rw[a] = 1.0; uw[a] = vw[a] = ww[a] = 0.0; Tw[a] = mw[a] = 1.0; Hw[a] = 0.0; }
   if (active) {
 #pragma unroll
-    for (int a = 3; a < 7; ++a) {          // planes k0-3 .. k0 sit in slots 3..6 at s = k0-3
+    for (int a = 3; a < 6; ++a) {          // planes k0-3 .. k0-1 sit in slots 3..5 at s = k0-3
       const double* q = qown + (size_t)map_z(P, k0 - 6 + a) * P.nxy;
       rw[a] = __ldg(q); uw[a] = __ldg(q + P.N); vw[a] = __ldg(q + 2 * P.N); ww[a] = __ldg(q + 3 * P.N);
       Tw[a] = __ldg(q + 4 * P.N); mw[a] = __ldg(q + 5 * P.N); Hw[a] = __ldg(q + 6 * P.N);
     }
   }
   // own node of the planes ahead: plane s+5 is requested at the top of step s (cp.async, thread-private
-  // slot, no register and no barrier), plane s+4 is taken from the ring at the end of step s
+  // slot, no register and no barrier) into ring slot (it+5) % 3; plane s+3 is read from slot it % 3
   const unsigned own0 = smem_u32(oring + tid);
-  if (active) {
-    const double* q = qown + (size_t)map_z(P, k0 + 1) * P.nxy;
 #pragma unroll
-    for (int f = 0; f < NF; ++f) cp_async8(own0 + ((1 * NF + f) * NPT) * 8, q + f * P.N);
+  for (int b = 0; b < 2; ++b) {
+    if (active) {
+      const double* q = qown + (size_t)map_z(P, k0 + b) * P.nxy;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) cp_async8(own0 + ((b * NF + f) * NPT) * 8, q + f * P.N);
+    }
+    cp_async_commit();
   }
-  cp_async_commit();
   const double dt = FUSED ? *A.dt_ptr : 0.0;
   int slot7 = 0, buf = 0;                                // it % 7, it % NBUF
   unsigned phase = 0;                                    // (it / NBUF) & 1
@@ -385,61 +442,47 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     double* t = tiles + buf * SM_TILE1;
     if (active && s + 5 < k1 + 3) {
       const double* q = qown + (size_t)map_z(P, s + 5) * P.nxy;
-      const unsigned d = own0 + ((it & 1) * NF * NPT) * 8;
+      const unsigned d = own0 + ((buf == 0 ? 2 : buf - 1) * NF * NPT) * 8;      // (it + 5) % 3
 #pragma unroll
       for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.N);
     }
     cp_async_commit();
+    cp_async_wait<2>();                                  // plane s+3 has landed (requested at step s-2)
+    const double* own3 = oring + buf * NF * NPT + tid;   // own node of plane s+3
     if (use_tma) mbar_wait(bar0 + 8 * buf, phase);
-    if (edge) {
-      fill_by_index(P, A.q, i0, j0, map_z(P, s), t, !use_tma, tid);
-      __syncthreads();
+    if (edge && it + 1 < nplanes) {
+      // ghost slots of the NEXT plane's tile: written before this step's barrier, read after it
+      const int b1 = buf == NBUF - 1 ? 0 : buf + 1;
+      if (use_tma && tid < npatch) mbar_wait(bar0 + 8 * b1, b1 == 0 ? phase ^ 1u : phase);
+      patch_tile(P, A.q, plist, npatch, map_z(P, s + 1), tiles + b1 * SM_TILE1, tid);
     }
-    // ---------------- in-plane derivatives shared through the staging rows -----------------------
     double* sgY = stg + (it & 1) * SM_STG1;
     double* sgX = sgY + SM_STGY;
-    const double dxu = d1_tile(P, t + F_U * TILE, oc, 1);
-    const double dyv = d1_tile(P, t + F_V * TILE, oc, PITCH);
-    sgX[(tj + HALO) * TX + ti] = dxu;
-    sgY[tj * PITCH + ti + XH] = dyv;
-    if (sj_dst >= 0) sgY[sj_dst] = d1_tile(P, t + sj_f * TILE, sj_src, sj_st);    // sgX follows sgY in memory
-    __syncthreads();
-    // every thread is past plane s-1: its buffer takes plane s+2
-    if (use_tma && tid == 0 && it + 2 < nplanes) {
-      const int b2 = buf == 0 ? 2 : buf - 1;             // (it + 2) % NBUF
-      fence_proxy_async();
-      mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
-      tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
-    }
+    if (sj_dst >= 0) sgY[sj_dst] = d1_tile(P, t, sj_src, sj_st);          // sgX follows sgY in memory
 
-    if (active) {
-      double g1, g2, g3;
-      if (!full) {
-        g1 = d1_tile(P, t + F_W * TILE, oc, 1) * ihx;
-        g2 = d1_tile(P, t + F_W * TILE, oc, PITCH) * ihy;
-        g3 = dxu * ihx + dyv * ihy;
-      } else {
+    NodeAcc N;
+    if (!active || !full) {
+      // ghost planes of the chunk, and tile nodes beyond the grid (their staging entries are the
+      // neighbours' ghost columns / rows): in-plane first derivatives only
+      const double dxu = d1_tile(P, t + F_U * TILE, oc, 1);
+      const double dyv = d1_tile(P, t + F_V * TILE, oc, PITCH);
+      sgX[(tj + HALO) * TX + ti] = dxu;
+      sgY[tj * PITCH + ti + XH] = dyv;
+      if (active) {
+        const double ihx = xi[ti], ihy = yi[tj];
+        double* gr = gring + slot7 * 3 * NPT + tid;
+        gr[0] = d1_tile(P, t + F_W * TILE, oc, 1) * ihx;
+        gr[NPT] = d1_tile(P, t + F_W * TILE, oc, PITCH) * ihy;
+        gr[2 * NPT] = dxu * ihx + dyv * ihy;
+      }
+    } else {
+      const double ihx = xi[ti], ihy = yi[tj];
+      {
         Nb c;
         c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
-        NodeAcc N;
 #pragma unroll
         for (int v = 0; v < 5; ++v) N.R[v] = 0.0;
         N.Va[0] = N.Va[1] = N.Va[2] = 0.0; N.LT = 0.0; N.heat = 0.0;
-        // ---- z, from the register windows ----
-        {
-          DirAcc Z;
-          acc_zero(Z);
-#pragma unroll
-          for (int l = 1; l <= 3; ++l) {
-            Nb p, m;
-            p.rho = rw[3 + l]; p.u = uw[3 + l]; p.v = vw[3 + l]; p.w = ww[3 + l]; p.T = Tw[3 + l]; p.mu = mw[3 + l]; p.H = Hw[3 + l];
-            m.rho = rw[3 - l]; m.u = uw[3 - l]; m.v = vw[3 - l]; m.w = ww[3 - l]; m.T = Tw[3 - l]; m.mu = mw[3 - l]; m.H = Hw[3 - l];
-            dir_accum<2>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Z);
-          }
-          double f[5];
-          conv_from_acc<2>(c, Z, f);
-          dir_fold<2>(P, c, Z, f, P.ih[2][s], P.gh[2][s], N);
-        }
         // ---- x ----
         {
           DirAcc X;
@@ -449,6 +492,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
             const Nb p = tile_nb(t, oc + l), m = tile_nb(t, oc - l);
             dir_accum<0>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, X);
           }
+          sgX[(tj + HALO) * TX + ti] = X.du;                                 // D_x u, for d_y(d_x u) of the neighbours
           double f[5];
           conv_from_acc<0>(c, X, f);
           if (gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) {
@@ -456,7 +500,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
           }
-          dir_fold<0>(P, c, X, f, ihx, ghx, N);
+          dir_fold<0>(P, c, X, f, ihx, xg[ti], N);
         }
         // ---- y ----
         {
@@ -467,6 +511,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
             const Nb p = tile_nb(t, oc + l * PITCH), m = tile_nb(t, oc - l * PITCH);
             dir_accum<1>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Y);
           }
+          sgY[tj * PITCH + ti + XH] = Y.dv;                                  // D_y v, for d_x(d_y v) of the neighbours
           double f[5];
           conv_from_acc<1>(c, Y, f);
           const bool wall_lo = gj == 0 && P.bc[2] == BC_WALL_STAG;
@@ -476,36 +521,53 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
           }
-          dir_fold<1>(P, c, Y, f, ihy, ghy, N);
+          dir_fold<1>(P, c, Y, f, ihy, yg[tj], N);
         }
-        g1 = N.G[6]; g2 = N.G[7]; g3 = N.G[0] + N.G[4];
-        if (P.viscous) {
-          // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
-          const int sy = tj * PITCH + ti + XH, sx = (tj + HALO) * TX + ti;
-          double mxy = P.c.a[0] * (sgY[sy + 1] - sgY[sy - 1]);
-          mxy = fma(P.c.a[1], sgY[sy + 2] - sgY[sy - 2], mxy);
-          mxy = fma(P.c.a[2], sgY[sy + 3] - sgY[sy - 3], mxy);
-          double myx = P.c.a[0] * (sgX[sx + TX] - sgX[sx - TX]);
-          myx = fma(P.c.a[1], sgX[sx + 2 * TX] - sgX[sx - 2 * TX], myx);
-          myx = fma(P.c.a[2], sgX[sx + 3 * TX] - sgX[sx - 3 * TX], myx);
-          const double ixy3 = ihx * ihy * (1.0 / 3.0);
-          N.Va[0] = fma(mxy, ixy3, N.Va[0]);
-          N.Va[1] = fma(myx, ixy3, N.Va[1]);
-          visc_assemble(P, c, N);
-        }
-        double* rr = rring + (it & 3) * 5 * NPT + tid;
-#pragma unroll
-        for (int v = 0; v < 5; ++v) rr[v * NPT] = N.R[v];
       }
       double* gr = gring + slot7 * 3 * NPT + tid;
-      gr[0] = g1; gr[NPT] = g2; gr[2 * NPT] = g3;
+      gr[0] = N.G[6]; gr[NPT] = N.G[7]; gr[2 * NPT] = N.G[0] + N.G[4];
+    }
+    // ---- the plane's barrier, first half: everything other threads read of this step is written ----
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(sbar);
+
+    if (active && full) {
+      // ---- z, from the register windows ----
+      Nb c;
+      c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
+      DirAcc Z;
+      acc_zero(Z);
+#pragma unroll
+      for (int l = 1; l <= 3; ++l) {
+        Nb p, m;
+        if (l < 3) {
+          p.rho = rw[3 + l]; p.u = uw[3 + l]; p.v = vw[3 + l]; p.w = ww[3 + l]; p.T = Tw[3 + l]; p.mu = mw[3 + l]; p.H = Hw[3 + l];
+        } else {
+          p.rho = own3[F_RHO * NPT]; p.u = own3[F_U * NPT]; p.v = own3[F_V * NPT]; p.w = own3[F_W * NPT];
+          p.T = own3[F_T * NPT]; p.mu = own3[F_MU * NPT]; p.H = own3[F_H * NPT];
+        }
+        m.rho = rw[3 - l]; m.u = uw[3 - l]; m.v = vw[3 - l]; m.w = ww[3 - l]; m.T = Tw[3 - l]; m.mu = mw[3 - l]; m.H = Hw[3 - l];
+        dir_accum<2>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Z);
+      }
+      double f[5];
+      conv_from_acc<2>(c, Z, f);
+      dir_fold<2>(P, c, Z, f, zi[s - k0], zg[s - k0], N);
+    }
+    // ---- second half of the barrier: the staging rows of this plane are complete ----
+    mbar_wait(sbar, (unsigned)(it & 1));
+    // every thread is past plane s-1: its buffer takes plane s+2
+    if (use_tma && tid == 0 && it + 2 < nplanes) {
+      const int b2 = buf == 0 ? 2 : buf - 1;             // (it + 2) % NBUF
+      fence_proxy_async();
+      mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
+      tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
     }
     // ================= plane p = s-3: add the z-mixed terms, write the result ====================
     const int p = s - 3;
     if (active && p >= k0) {
       double R[5];
       {
-        const double* rr = rring + ((it - 3) & 3) * 5 * NPT + tid;
+        const double* rr = rring + buf * 5 * NPT + tid;              // plane s-3 sits in slot it % 3
 #pragma unroll
         for (int v = 0; v < 5; ++v) R[v] = rr[v * NPT];
       }
@@ -522,12 +584,12 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
 #pragma unroll
           for (int m = 0; m < 3; ++m) dz[m] = fma(a, gp[m * NPT] - gn[m * NPT], dz[m]);
         }
-        const double f3 = mw[0] * (1.0 / 3.0) * P.ih[2][p];
+        const double f3 = mw[0] * (1.0 / 3.0) * zi[p - k0];
         const double v0 = f3 * dz[0], v1 = f3 * dz[1], v2 = f3 * dz[2];
         R[1] += v0; R[2] += v1; R[3] += v2;
         R[4] += uw[0] * v0 + vw[0] * v1 + ww[0] * v2;
       }
-      fsum += R[1] * (hxy * P.hh[2][p]);
+      fsum = fma(R[1], zh[p - k0], fsum);                                      // times h_x h_y after the loop
       // ---------------- epilogue: write R, or the RK3 stage of Eq. 11 ------------------------------
       const size_t o = (size_t)p * P.nxy + own_off;
       if (!FUSED) {
@@ -549,22 +611,42 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
         A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 5 * P.N] = qn.mu; A.q_out[o + 6 * P.N] = qn.H;
       }
     }
+    if (active && full) {
+      if (P.viscous) {
+        // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
+        const int sy = tj * PITCH + ti + XH, sx = (tj + HALO) * TX + ti;
+        double mxy = P.c.a[0] * (sgY[sy + 1] - sgY[sy - 1]);
+        mxy = fma(P.c.a[1], sgY[sy + 2] - sgY[sy - 2], mxy);
+        mxy = fma(P.c.a[2], sgY[sy + 3] - sgY[sy - 3], mxy);
+        double myx = P.c.a[0] * (sgX[sx + TX] - sgX[sx - TX]);
+        myx = fma(P.c.a[1], sgX[sx + 2 * TX] - sgX[sx - 2 * TX], myx);
+        myx = fma(P.c.a[2], sgX[sx + 3 * TX] - sgX[sx - 3 * TX], myx);
+        const double ixy3 = xi[ti] * yi[tj] * (1.0 / 3.0);
+        N.Va[0] = fma(mxy, ixy3, N.Va[0]);
+        N.Va[1] = fma(myx, ixy3, N.Va[1]);
+        Nb c;
+        c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
+        visc_assemble(P, c, N);
+      }
+      double* rr = rring + buf * 5 * NPT + tid;
+#pragma unroll
+      for (int v = 0; v < 5; ++v) rr[v * NPT] = N.R[v];
+    }
     slot7 = slot7 == 6 ? 0 : slot7 + 1;
     if (++buf == NBUF) { buf = 0; phase ^= 1u; }
     // ---------------- shift the windows, own node of plane s+4 ------------------------------------
 #pragma unroll
-    for (int a = 0; a < 6; ++a) {
+    for (int a = 0; a < 5; ++a) {
       rw[a] = rw[a + 1]; uw[a] = uw[a + 1]; vw[a] = vw[a + 1]; ww[a] = ww[a + 1]; Tw[a] = Tw[a + 1]; mw[a] = mw[a + 1]; Hw[a] = Hw[a + 1];
     }
-    cp_async_wait<1>();                                  // plane s+4 has landed (requested at step s-1)
-    if (active && s + 4 < k1 + 3) {
-      const double* o = oring + ((it + 1) & 1) * NF * NPT + tid;
-      rw[6] = o[F_RHO * NPT]; uw[6] = o[F_U * NPT]; vw[6] = o[F_V * NPT]; ww[6] = o[F_W * NPT];
-      Tw[6] = o[F_T * NPT]; mw[6] = o[F_MU * NPT]; Hw[6] = o[F_H * NPT];
+    if (active && s + 3 < k1 + 3) {
+      rw[5] = own3[F_RHO * NPT]; uw[5] = own3[F_U * NPT]; vw[5] = own3[F_V * NPT]; ww[5] = own3[F_W * NPT];
+      Tw[5] = own3[F_T * NPT]; mw[5] = own3[F_MU * NPT]; Hw[5] = own3[F_H * NPT];
     }
   }
   if (A.partial) {
-    const double tot = block_sum<NT>(fsum, red, tid);
+    const double hxy = active ? P.hh[0][gi] * P.hh[1][gj] : 0.0;
+    const double tot = block_sum<NT>(fsum * hxy, red, tid);
     if (tid == 0) A.partial[(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = tot;
   }
 }
