@@ -69,6 +69,31 @@ __global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, d
   }
 }
 
+// ---- lazy forcing (S9 with Eq. 11): the fused k_rhs<true> advanced the state WITHOUT this stage's body force (f is
+// only known once the whole R has been summed); this adds dt beta f (e_rhou + u e_rhoE), u = the velocity of the
+// stage's input state `Qin`, to the new state `Q` (rho, v, w are not touched).  Same map as advance_prim.
+__global__ void __launch_bounds__(RT) k_force_fix(const __grid_constant__ DevP P, double* __restrict__ Q, const double* __restrict__ Qin,
+                                                  const DevScal* __restrict__ sc, double beta) {
+  const double c = sc->dt * beta * sc->force;
+  const bool wn0 = P.bc[2] == BC_WALL_NODE, wn1 = P.bc[3] == BC_WALL_NODE;
+  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
+    if (wn0 || wn1) {
+      const int j = (int)((o / P.nx) % P.ny);
+      if ((wn0 && j == 0) || (wn1 && j == P.ny - 1)) continue;      // Dirichlet wall node: already overridden
+    }
+    const double rho = Q[o], u = Q[o + P.N], T = Q[o + 4 * P.N], H = Q[o + 6 * P.N];
+    const double ul = Qin[o + P.N];
+    const double ir = 1.0 / rho;
+    const double du = c * ir, dE = (c * ul) * ir;
+    const double un = u + du;
+    const double dke = 0.5 * (du * (un + u));
+    const double dT = (dE - dke) * P.inv_cv;
+    const double Tn = T + dT;
+    Q[o + P.N] = un; Q[o + 4 * P.N] = Tn; Q[o + 5 * P.N] = visc_mu(P, Tn);
+    Q[o + 6 * P.N] = H + fma(P.cp, dT, dke);
+  }
+}
+
 // R_rhou += f, R_rhoE += f u  (streams_rhs with forcing)
 __global__ void __launch_bounds__(RT) k_apply_force(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ R,
                                                     const DevScal* __restrict__ sc) {

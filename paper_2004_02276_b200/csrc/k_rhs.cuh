@@ -39,7 +39,8 @@ constexpr int TILE = PY * PITCH;                // doubles per tile field (560)
 enum { F_RHO = 0, F_U, F_V, F_W, F_T, F_MU, F_H, NF };   // = order of the fields of Q
 static_assert(NF == NQ, "tile fields are the stored primitives");
 
-constexpr int NBUF = 3;                         // tile ring: plane s is used while s+1, s+2 are in flight
+constexpr int NBUF = 2;                         // tile buffers: plane s is used while s+1 lands; s+2 is requested into the
+                                                // buffer of plane s once every thread is past its in-plane reads (step barrier)
 constexpr int SM_TILE1 = NF * TILE;             // one plane (3920 doubles = 31360 B, a multiple of 128 B)
 constexpr int SM_TILES = NBUF * SM_TILE1;
 constexpr int SM_STGY = TY * PITCH;             // D_y v on the x-extended rows
@@ -49,11 +50,12 @@ constexpr int SM_GRING = 7 * 3 * NPT;
 constexpr int SM_RRING = 3 * 5 * NPT;     // R of planes s-1..s-3: read (plane s-3) before written (plane s) in a step
 constexpr int NOWN = 3;                         // own-node ring: plane s+3 is read while s+4, s+5 are in flight
 constexpr int SM_OWN = NOWN * NF * NPT;
+constexpr int SM_SPREV = 6 * NPT;                // FUSED: R_prev (5) and u_prev of plane s-3, prefetched by cp.async
 constexpr int SM_RED = 32;
 constexpr int LZ_MAX = 128;                     // planes per CTA (make_layout caps the chunk length)
 constexpr int SM_MET = 3 * LZ_MAX + 2 * TX + 2 * TY;   // 1/h_z, -g_z/h_z^3, h_z of the chunk; 1/h, -g/h^3 of the tile's x and y
 constexpr int SM_PATCH = TILE;                  // ghost-slot list of an edge tile: one int2 (8 bytes) per entry
-constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_MET + SM_PATCH + SM_RED + 8;
+constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_SPREV + SM_MET + SM_PATCH + SM_RED + 8;
 static_assert(SM_RHS_DOUBLES * 8 <= 227 * 1024, "one CTA per SM: the shared-memory budget of sm_100a");
 constexpr int NSTAGE = 2 * HALO * TY + 2 * HALO * TX;                     // 240 staged derivatives outside the tile
 constexpr unsigned TILE_BYTES = SM_TILE1 * sizeof(double);
@@ -66,6 +68,9 @@ struct RhsArgs {
   const double* S_prev;   // FUSED: R of the previous stage (ignored when alpha == 0)
   double* S_out;          // FUSED: R of this stage (may alias S_prev)
   const double* dt_ptr;   // FUSED: time step on the device
+  const double* f_prev;   // FUSED, lazy forcing (S9): body force of the previous stage, or NULL.  S_prev then holds the
+                          // previous R WITHOUT its forcing terms; they are added here as f_prev (e_rhou + u_prev e_rhoE),
+                          // u_prev = the velocity still sitting in q_out (the previous stage's input state)
   double alpha, beta;
   double* partial;        // per-CTA partial sums of R_rhou * vol (forcing), may be NULL
   int lz;                 // planes per CTA
@@ -325,7 +330,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   double* gring = stg + 2 * SM_STG1;
   double* rring = gring + SM_GRING;
   double* oring = rring + SM_RRING;
-  double* met = oring + SM_OWN;
+  double* spring = oring + SM_OWN;
+  double* met = spring + SM_SPREV;
   int2* plist = reinterpret_cast<int2*>(met + SM_MET);
   double* red = met + SM_MET + SM_PATCH;
   const unsigned bar0 = smem_u32(red + SM_RED);          // NBUF mbarriers: tile buffer b holds its plane
@@ -397,18 +403,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
 
   double fsum = 0.0;
 
-  // staged derivative outside the tile: [0,48) D_y v on the x-halo columns, [48,240) D_x u on the y-halo rows
-  int sj_src = 0, sj_dst = -1, sj_st = 1;
-  if (tid < 2 * HALO * TY) {
-    const int r = tid / 6, c = tid % 6, io = c < 3 ? c - 3 : TX + c - 3;
-    sj_src = F_V * TILE + (r + HALO) * PITCH + io + XH; sj_dst = r * PITCH + io + XH; sj_st = PITCH;
-  } else if (tid < NSTAGE) {
-    const int e2 = tid - 2 * HALO * TY, rr = e2 / TX, col = e2 % TX, jo = rr < 3 ? rr - 3 : TY + rr - 3;
-    sj_src = F_U * TILE + (jo + HALO) * PITCH + col + XH; sj_dst = SM_STGY + (jo + HALO) * TX + col; sj_st = 1;
-  }
-
   // register windows of the own node: index a holds plane s-3+a
-  const double* qown = A.q + own_off;
   // (plane s+3 stays in the own-node ring: read for the l = 3 pair and again when it enters the window)
   double rw[6], uw[6], vw[6], ww[6], Tw[6], mw[6], Hw[6];
 #pragma unroll
@@ -416,67 +411,92 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   if (active) {
 #pragma unroll
     for (int a = 3; a < 6; ++a) {          // planes k0-3 .. k0-1 sit in slots 3..5 at s = k0-3
-      const double* q = qown + (size_t)map_z(P, k0 - 6 + a) * P.nxy;
+      const double* q = A.q + own_off + (size_t)map_z(P, k0 - 6 + a) * P.nxy;
       rw[a] = __ldg(q); uw[a] = __ldg(q + P.N); vw[a] = __ldg(q + 2 * P.N); ww[a] = __ldg(q + 3 * P.N);
       Tw[a] = __ldg(q + 4 * P.N); mw[a] = __ldg(q + 5 * P.N); Hw[a] = __ldg(q + 6 * P.N);
     }
   }
   // own node of the planes ahead: plane s+5 is requested at the top of step s (cp.async, thread-private
   // slot, no register and no barrier) into ring slot (it+5) % 3; plane s+3 is read from slot it % 3
-  const unsigned own0 = smem_u32(oring + tid);
 #pragma unroll
   for (int b = 0; b < 2; ++b) {
     if (active) {
-      const double* q = qown + (size_t)map_z(P, k0 + b) * P.nxy;
+      const double* q = A.q + own_off + (size_t)map_z(P, k0 + b) * P.nxy;
 #pragma unroll
-      for (int f = 0; f < NF; ++f) cp_async8(own0 + ((b * NF + f) * NPT) * 8, q + f * P.N);
+      for (int f = 0; f < NF; ++f) cp_async8(smem_u32(oring + tid) + ((b * NF + f) * NPT) * 8, q + f * P.N);
     }
     cp_async_commit();
   }
-  const double dt = FUSED ? *A.dt_ptr : 0.0;
-  int slot7 = 0, buf = 0;                                // it % 7, it % NBUF
-  unsigned phase = 0;                                    // (it / NBUF) & 1
+  // dt and the previous stage's body force sit in shared memory (read once per plane in the epilogue)
+  double* scal = red + SM_RED + NBUF + 2;
+  if (FUSED && tid == 0) {
+    scal[0] = *A.dt_ptr;
+    scal[1] = A.f_prev && A.alpha != 0.0 ? *A.f_prev : 0.0;
+  }
+  __syncthreads();
+  int slot7 = 0, b3 = 0;                                 // it % 7, it % 3
 
   for (int s = k0 - 3, it = 0; s < k1 + 3; ++s, ++it) {
     const bool full = s >= k0 && s < k1;
+    const int buf = it & 1;                              // tile buffer of plane s; its mbarrier is in phase (it >> 1) & 1
+    const unsigned phase = (unsigned)(it >> 1) & 1u;
     double* t = tiles + buf * SM_TILE1;
     if (active && s + 5 < k1 + 3) {
-      const double* q = qown + (size_t)map_z(P, s + 5) * P.nxy;
-      const unsigned d = own0 + ((buf == 0 ? 2 : buf - 1) * NF * NPT) * 8;      // (it + 5) % 3
+      const double* q = A.q + own_off + (size_t)map_z(P, s + 5) * P.nxy;
+      const unsigned d = smem_u32(oring + tid) + ((b3 == 0 ? 2 : b3 - 1) * NF * NPT) * 8;       // (it + 5) % 3
 #pragma unroll
       for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.N);
     }
+    if (FUSED && A.alpha != 0.0 && active && s - 3 >= k0) {
+      // R_prev (and u_prev for the lazy forcing) of plane s-3, read in this step's epilogue
+      const size_t o = (size_t)(s - 3) * P.nxy + own_off;
+      const unsigned d = smem_u32(spring + tid);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) cp_async8(d + v * NPT * 8, A.S_prev + o + v * P.N);
+      if (A.f_prev) cp_async8(d + 5 * NPT * 8, A.q_out + o + P.N);
+    }
     cp_async_commit();
     cp_async_wait<2>();                                  // plane s+3 has landed (requested at step s-2)
-    const double* own3 = oring + buf * NF * NPT + tid;   // own node of plane s+3
+    int tl = tid;                                        // opaque copy: keeps per-thread shared-memory addresses from being
+    asm volatile("" : "+r"(tl));                         // hoisted out of the loop (and then spilled) instead of recomputed
+    const int li = tl & (TX - 1), lj = tl / TX, loc = (lj + HALO) * PITCH + li + XH;
+    const double* own3 = oring + b3 * NF * NPT + tl;     // own node of plane s+3
     if (use_tma) mbar_wait(bar0 + 8 * buf, phase);
     if (edge && it + 1 < nplanes) {
       // ghost slots of the NEXT plane's tile: written before this step's barrier, read after it
-      const int b1 = buf == NBUF - 1 ? 0 : buf + 1;
-      if (use_tma && tid < npatch) mbar_wait(bar0 + 8 * b1, b1 == 0 ? phase ^ 1u : phase);
-      patch_tile(P, A.q, plist, npatch, map_z(P, s + 1), tiles + b1 * SM_TILE1, tid);
+      const int b1 = buf ^ 1;
+      if (use_tma && tl < npatch) mbar_wait(bar0 + 8 * b1, (unsigned)((it + 1) >> 1) & 1u);
+      patch_tile(P, A.q, plist, npatch, map_z(P, s + 1), tiles + b1 * SM_TILE1, tl);
     }
     double* sgY = stg + (it & 1) * SM_STG1;
     double* sgX = sgY + SM_STGY;
-    if (sj_dst >= 0) sgY[sj_dst] = d1_tile(P, t, sj_src, sj_st);          // sgX follows sgY in memory
+    // staged derivative outside the tile: threads [0,48) D_y v on the x-halo columns, [48,240) D_x u on the y-halo rows
+    // (indices recomputed every plane: cheaper than three registers carried through the loop)
+    if (tl < 2 * HALO * TY) {
+      const int r = tl / 6, c = tl % 6, io = c < 3 ? c - 3 : TX + c - 3;
+      sgY[r * PITCH + io + XH] = d1_tile(P, t + F_V * TILE, (r + HALO) * PITCH + io + XH, PITCH);
+    } else if (tl < NSTAGE) {
+      const int e2 = tl - 2 * HALO * TY, rr = e2 / TX, col = e2 % TX, jo = rr < 3 ? rr - 3 : TY + rr - 3;
+      sgX[(jo + HALO) * TX + col] = d1_tile(P, t + F_U * TILE, (jo + HALO) * PITCH + col + XH, 1);
+    }
 
     NodeAcc N;
     if (!active || !full) {
       // ghost planes of the chunk, and tile nodes beyond the grid (their staging entries are the
       // neighbours' ghost columns / rows): in-plane first derivatives only
-      const double dxu = d1_tile(P, t + F_U * TILE, oc, 1);
-      const double dyv = d1_tile(P, t + F_V * TILE, oc, PITCH);
-      sgX[(tj + HALO) * TX + ti] = dxu;
-      sgY[tj * PITCH + ti + XH] = dyv;
+      const double dxu = d1_tile(P, t + F_U * TILE, loc, 1);
+      const double dyv = d1_tile(P, t + F_V * TILE, loc, PITCH);
+      sgX[(lj + HALO) * TX + li] = dxu;
+      sgY[lj * PITCH + li + XH] = dyv;
       if (active) {
-        const double ihx = xi[ti], ihy = yi[tj];
-        double* gr = gring + slot7 * 3 * NPT + tid;
-        gr[0] = d1_tile(P, t + F_W * TILE, oc, 1) * ihx;
-        gr[NPT] = d1_tile(P, t + F_W * TILE, oc, PITCH) * ihy;
+        const double ihx = xi[li], ihy = yi[lj];
+        double* gr = gring + slot7 * 3 * NPT + tl;
+        gr[0] = d1_tile(P, t + F_W * TILE, loc, 1) * ihx;
+        gr[NPT] = d1_tile(P, t + F_W * TILE, loc, PITCH) * ihy;
         gr[2 * NPT] = dxu * ihx + dyv * ihy;
       }
     } else {
-      const double ihx = xi[ti], ihy = yi[tj];
+      const double ihx = xi[li], ihy = yi[lj];
       {
         Nb c;
         c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
@@ -489,18 +509,18 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
           acc_zero(X);
 #pragma unroll
           for (int l = 1; l <= 3; ++l) {
-            const Nb p = tile_nb(t, oc + l), m = tile_nb(t, oc - l);
+            const Nb p = tile_nb(t, loc + l), m = tile_nb(t, loc - l);
             dir_accum<0>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, X);
           }
-          sgX[(tj + HALO) * TX + ti] = X.du;                                 // D_x u, for d_y(d_x u) of the neighbours
+          sgX[(lj + HALO) * TX + li] = X.du;                                 // D_x u, for d_y(d_x u) of the neighbours
           double f[5];
           conv_from_acc<0>(c, X, f);
           if (gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) {
-            const F5 r = outflow_x(P, t, oc);
+            const F5 r = outflow_x(P, t, loc);
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
           }
-          dir_fold<0>(P, c, X, f, ihx, xg[ti], N);
+          dir_fold<0>(P, c, X, f, ihx, xg[li], N);
         }
         // ---- y ----
         {
@@ -508,28 +528,28 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
           acc_zero(Y);
 #pragma unroll
           for (int l = 1; l <= 3; ++l) {
-            const Nb p = tile_nb(t, oc + l * PITCH), m = tile_nb(t, oc - l * PITCH);
+            const Nb p = tile_nb(t, loc + l * PITCH), m = tile_nb(t, loc - l * PITCH);
             dir_accum<1>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Y);
           }
-          sgY[tj * PITCH + ti + XH] = Y.dv;                                  // D_y v, for d_x(d_y v) of the neighbours
+          sgY[lj * PITCH + li + XH] = Y.dv;                                  // D_y v, for d_x(d_y v) of the neighbours
           double f[5];
           conv_from_acc<1>(c, Y, f);
           const bool wall_lo = gj == 0 && P.bc[2] == BC_WALL_STAG;
           const bool wall_hi = gj == P.ny - 1 && P.bc[3] == BC_WALL_STAG;
           if (wall_lo || wall_hi) {
-            const F5 r = wall_y(P, t, oc, wall_lo, wall_hi);
+            const F5 r = wall_y(P, t, loc, wall_lo, wall_hi);
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
           }
-          dir_fold<1>(P, c, Y, f, ihy, yg[tj], N);
+          dir_fold<1>(P, c, Y, f, ihy, yg[lj], N);
         }
       }
-      double* gr = gring + slot7 * 3 * NPT + tid;
+      double* gr = gring + slot7 * 3 * NPT + tl;
       gr[0] = N.G[6]; gr[NPT] = N.G[7]; gr[2 * NPT] = N.G[0] + N.G[4];
     }
     // ---- the plane's barrier, first half: everything other threads read of this step is written ----
     __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive(sbar);
+    if ((tl & 31) == 0) mbar_arrive(sbar);
 
     if (active && full) {
       // ---- z, from the register windows ----
@@ -555,9 +575,9 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     }
     // ---- second half of the barrier: the staging rows of this plane are complete ----
     mbar_wait(sbar, (unsigned)(it & 1));
-    // every thread is past plane s-1: its buffer takes plane s+2
-    if (use_tma && tid == 0 && it + 2 < nplanes) {
-      const int b2 = buf == 0 ? 2 : buf - 1;             // (it + 2) % NBUF
+    // every thread is past its reads of this plane's tile: the buffer takes plane s+2
+    if (use_tma && tl == 0 && it + 2 < nplanes) {
+      const int b2 = buf;                                // (it + 2) % NBUF
       fence_proxy_async();
       mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
       tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
@@ -567,7 +587,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     if (active && p >= k0) {
       double R[5];
       {
-        const double* rr = rring + buf * 5 * NPT + tid;              // plane s-3 sits in slot it % 3
+        const double* rr = rring + b3 * 5 * NPT + tl;               // plane s-3 sits in slot it % 3
 #pragma unroll
         for (int v = 0; v < 5; ++v) R[v] = rr[v * NPT];
       }
@@ -578,8 +598,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
         for (int l = 1; l <= 3; ++l) {
           int sp = slot7 - 3 + l; if (sp < 0) sp += 7;
           int sn = slot7 - 3 - l; if (sn < 0) sn += 7;
-          const double* gp = gring + sp * 3 * NPT + tid;
-          const double* gn = gring + sn * 3 * NPT + tid;
+          const double* gp = gring + sp * 3 * NPT + tl;
+          const double* gn = gring + sn * 3 * NPT + tl;
           const double a = P.c.a[l - 1];
 #pragma unroll
           for (int m = 0; m < 3; ++m) dz[m] = fma(a, gp[m * NPT] - gn[m * NPT], dz[m]);
@@ -597,9 +617,14 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
         for (int v = 0; v < 5; ++v) A.out_rhs[o + v * P.N] = R[v];
       } else {
         double dW[5];
+        const double dt = scal[0], fprev = scal[1];
+        cp_async_wait<0>();                              // R_prev / u_prev of this plane (requested at the top of the step)
+        const double* pv = spring + tl;
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
-          const double sp = A.alpha != 0.0 ? A.S_prev[o + v * P.N] : 0.0;
+          double sp = A.alpha != 0.0 ? pv[v * NPT] : 0.0;
+          if (v == 1) sp += fprev;
+          if (v == 4 && A.f_prev && A.alpha != 0.0) sp = fma(fprev, pv[5 * NPT], sp);
           dW[v] = dt * (A.alpha * sp + A.beta * R[v]);
           A.S_out[o + v * P.N] = R[v];
         }
@@ -614,26 +639,26 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     if (active && full) {
       if (P.viscous) {
         // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
-        const int sy = tj * PITCH + ti + XH, sx = (tj + HALO) * TX + ti;
+        const int sy = lj * PITCH + li + XH, sx = (lj + HALO) * TX + li;
         double mxy = P.c.a[0] * (sgY[sy + 1] - sgY[sy - 1]);
         mxy = fma(P.c.a[1], sgY[sy + 2] - sgY[sy - 2], mxy);
         mxy = fma(P.c.a[2], sgY[sy + 3] - sgY[sy - 3], mxy);
         double myx = P.c.a[0] * (sgX[sx + TX] - sgX[sx - TX]);
         myx = fma(P.c.a[1], sgX[sx + 2 * TX] - sgX[sx - 2 * TX], myx);
         myx = fma(P.c.a[2], sgX[sx + 3 * TX] - sgX[sx - 3 * TX], myx);
-        const double ixy3 = xi[ti] * yi[tj] * (1.0 / 3.0);
+        const double ixy3 = xi[li] * yi[lj] * (1.0 / 3.0);
         N.Va[0] = fma(mxy, ixy3, N.Va[0]);
         N.Va[1] = fma(myx, ixy3, N.Va[1]);
         Nb c;
         c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
         visc_assemble(P, c, N);
       }
-      double* rr = rring + buf * 5 * NPT + tid;
+      double* rr = rring + b3 * 5 * NPT + tl;
 #pragma unroll
       for (int v = 0; v < 5; ++v) rr[v * NPT] = N.R[v];
     }
     slot7 = slot7 == 6 ? 0 : slot7 + 1;
-    if (++buf == NBUF) { buf = 0; phase ^= 1u; }
+    b3 = b3 == 2 ? 0 : b3 + 1;
     // ---------------- shift the windows, own node of plane s+4 ------------------------------------
 #pragma unroll
     for (int a = 0; a < 5; ++a) {

@@ -526,7 +526,18 @@ int streams_step(streams_ctx* c, int nsteps) {
       RhsArgs A;
       std::memset(&A, 0, sizeof A);
       A.q = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
-      if (c->p.forcing) {
+      if (c->p.forcing && !c->p.weno_enable) {
+        // lazy forcing: the fused kernel advances with alpha (R_prev + f_prev ...) + beta R and sums R_rhou; once f is
+        // known a light kernel adds dt beta f (e_rhou + u e_rhoE).  S[0] keeps R without the forcing terms.
+        double* wn = c->qbuf[c->cur ^ 1];
+        A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
+        A.f_prev = l > 0 ? &c->sc->force : nullptr;
+        if ((rc = launch_rhs(c, true, A))) return rc;
+        if ((rc = force_from_partials(c, nullptr, true))) return rc;
+        k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l]);
+        LAUNCH_CHECK("k_force_fix");
+        c->cur ^= 1;
+      } else if (c->p.forcing) {
         // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
         double* Sp = c->S[c->scur];
         double* Sc = c->S[c->scur ^ 1];
