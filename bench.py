@@ -49,11 +49,20 @@ def make_workload(cfg: int, scale: float = 1.0):
 
 
 def bytes_per_point_per_launch(params) -> int:
-    """Algorithmic HBM bytes per grid point of ONE k_rhs launch."""
-    if params["forcing"]:
-        return 80            # read w (40 B) + write R (40 B); the update is a separate kernel
-    # fused RK stage: read w, write w', read S (stages 1,2), write S (the last stage's S write is dead but done)
-    return 160
+    """Algorithmic HBM bytes per grid point of ONE fused k_rhs launch."""
+    if params["forcing"] and params["weno_enable"]:
+        return 80            # unfused fallback: read w (40 B) + write R (40 B); the update is a separate kernel
+    # fused RK stage: read w, write w', read R_prev, write R (SURVEY 8.d: 160 B/point/stage; the read of R_prev is
+    # skipped in stage 0 and the write of R is dead in stage 2, both counted); lazy forcing adds u_prev (8 B) here
+    # and 8 B in the fix kernel, counted here as 16 B (SURVEY H-note 2: 176 B/point/stage)
+    return 176 if params["forcing"] else 160
+
+
+# fp64 work of ONE k_rhs launch per grid point (DESIGN.md section 6: hand count of the kernel's arithmetic without
+# the ghost planes of a chunk, cross-checked against ncu's executed DFMA/DADD/DMUL counts)
+DP_INSTR_RHS, DP_FLOP_RHS = 552, 826          # residual only (streams_rhs; unfused fallback)
+DP_INSTR_STAGE, DP_FLOP_STAGE = 111, 170      # + the fused RK stage: Eq. 11, primitives of the new state incl. mu(T)
+FP64_LANES_PER_SM, N_SM = 64, 148             # B200: fp64 lane-instructions per SM per clock (ncu peak_sustained = 64)
 
 
 def peaks():
@@ -209,6 +218,8 @@ def run_ours(args, rank, world, local_rank):
     ms_max = 1e3 * replicas.max_over_ranks(ms * 1e-3, dev)
     value = replicas.aggregate_throughput(npts, args.steps, ms * 1e-3, dev)
     diag = s.diagnostics(check=False)
+    from paper_2004_02276_b200.binding import fp64_peak
+    fp64_meas = 2.0 * fp64_peak() if rank == 0 else None                    # TFLOP/s (FMA = 2), measured live
 
     # ---- end to end through the C-ABI with HOST buffers ----------------------------------
     e2e = None
@@ -242,11 +253,17 @@ def run_ours(args, rank, world, local_rank):
         if os.path.exists(tpath):
             with open(tpath) as f:
                 traffic = json.load(f).get(wl.name)
-        step_bytes = {True: 3 * (80 + 176) + 40, False: 3 * 160 + 40}[bool(wl.params["forcing"])]
+        fused = not (wl.params["forcing"] and wl.params["weno_enable"])
+        step_bytes = 3 * bpp + 40 if fused else 3 * (80 + 176) + 40       # + the CFL pass over u, v, w, T
         cpu = None
         if not args.no_cpu:
             r = oracle_sample(wl, 1, planes=args.ref_planes)
             cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+        dp_instr = DP_INSTR_RHS + (DP_INSTR_STAGE if fused else 0)
+        dp_flop = DP_FLOP_RHS + (DP_FLOP_STAGE if fused else 0)
+        sm_clk = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
+        alu_peak = 2.0 * FP64_LANES_PER_SM * N_SM * sm_clk / 1e12           # TFLOP/s, FMA = 2 flop
+        alu_achieved = dp_flop * npts / (rhs_avg_ms * 1e-3) / 1e12
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f64", "data": "synthetic",
@@ -256,11 +273,17 @@ def run_ours(args, rank, world, local_rank):
                           "l2": "state (10.7 GB) and RK register larger than the 126 MB L2; no flush needed"
                           if state_bytes > 2 * 126e6 else "inputs smaller than L2 (launch-latency regime)"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-               "roofline": {"bound": "hbm", "kernel": "k_rhs", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                            "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                            "bytes_per_point_per_launch": bpp, "launches_timed": int(rhs_n), "avg_launch_ms": rhs_avg_ms,
+               "roofline": {"bound": "alu", "kernel": "k_rhs", "achieved": alu_achieved, "peak": alu_peak, "unit": "TFLOP/s",
+                            "frac": alu_achieved / alu_peak, "traffic": traffic,
+                            "peak_source": "fp64 FMA pipe: 148 SMs x 64 lanes x 2 flop x max SM clock (DESIGN.md section 6)",
+                            "peak_measured_TFLOPs": fp64_meas, "flop_per_point_per_launch": dp_flop,
+                            "fp64_instr_per_point_per_launch": dp_instr,
+                            "pipe_slot_frac": dp_instr * npts / (rhs_avg_ms * 1e-3) / (FP64_LANES_PER_SM * N_SM * sm_clk),
+                            "launches_timed": int(rhs_n), "avg_launch_ms": rhs_avg_ms,
                             "share_of_step": rhs_ms / ms if ms > 0 else None,
-                            "step_algorithmic_GBps": step_bytes * npts * args.steps / (ms_max * 1e-3) / 1e9},
+                            "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                                    "peak_source": peak_src, "bytes_per_point_per_launch": bpp,
+                                    "step_algorithmic_GBps": step_bytes * npts * args.steps / (ms_max * 1e-3) / 1e9}},
                "cpu_baseline": cpu,
                "state": {"time": diag.time, "dt": diag.dt, "min_rho": diag.min_rho, "nonfinite": int(diag.nonfinite)},
                "context": PAPER_CONTEXT}

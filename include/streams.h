@@ -157,6 +157,13 @@ int streams_diagnostics(streams_ctx* ctx, streams_diag* h_out);
 int streams_profile(streams_ctx* ctx, int enable);
 int streams_profile_read(streams_ctx* ctx, double* h_ms_total, long long* h_launches);
 
+/* Roofline denominator of an fp64-ALU-bound kernel: runs a register-only kernel of independent DFMA
+ * chains (one CTA of 1024 threads x 2 per SM) on `cuda_stream` (may be NULL = default stream) and
+ * returns in *h_tinstr the measured rate of fp64 lane-instructions in 1e12 per second (one DFMA of
+ * one thread = one; multiply by 2 for flop/s).  Nominal: 148 SMs x 64 lanes x SM clock.  Synchronises.
+ * Not part of the method (PAPER.md gives no peak); used by bench.py next to MEASURED_PEAKS.json. */
+int streams_fp64_peak(void* cuda_stream, double* h_tinstr);
+
 /* Number of kernel launches enqueued by this context so far (for bench accounting). */
 long long streams_launch_count(const streams_ctx* ctx);
 

@@ -74,6 +74,7 @@ def lib():
         L.streams_diagnostics.argtypes = [C.c_void_p, C.POINTER(StreamsDiag)]
         L.streams_profile.argtypes = [C.c_void_p, C.c_int]
         L.streams_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.streams_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.streams_launch_count.argtypes = [C.c_void_p]
         L.streams_launch_count.restype = C.c_longlong
         L.streams_last_error.argtypes = [C.c_void_p]
@@ -82,6 +83,15 @@ def lib():
         L.streams_destroy.restype = None
         _lib = L
     return _lib
+
+
+def fp64_peak(stream=None) -> float:
+    """Measured fp64 lane-instruction rate of the device in 1e12/s (include/streams.h: streams_fp64_peak)."""
+    v = C.c_double(0.0)
+    rc = lib().streams_fp64_peak(C.c_void_p(stream or 0), C.byref(v))
+    if rc != 0:
+        raise StreamsError(rc, lib().streams_last_error(None).decode())
+    return v.value
 
 
 def make_params(params: dict) -> StreamsParams:

@@ -186,6 +186,20 @@ __global__ void __launch_bounds__(RT) k_diag_partial(const __grid_constant__ Dev
   t = block_max<RT>(bad, sh, threadIdx.x);   if (threadIdx.x == 0) partial[10 * gridDim.x + blockIdx.x] = t;
 }
 
+// ---- fp64 pipe peak: 8 independent DFMA chains per thread, registers only (streams_fp64_peak) ----
+__global__ void __launch_bounds__(1024) k_fp64_peak(double* __restrict__ out, int iters, double a, double b) {
+  double x0 = threadIdx.x, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0, x7 = x0 + 7.0;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  const double r = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (r == 123.456) out[0] = r;              // never true: keeps the chains alive
+}
+
 // capture the frozen inflow plane (S1 INFLOW_FROZEN): inflow[v][k][j] = Q[v][k][j][0]
 __global__ void k_capture_inflow(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ inflow) {
   const long long n = (long long)P.nz * P.ny;

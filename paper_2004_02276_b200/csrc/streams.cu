@@ -221,6 +221,36 @@ const char* streams_last_error(const streams_ctx* c) { return c ? c->err : g_err
 
 long long streams_launch_count(const streams_ctx* c) { return c ? c->launches : 0; }
 
+int streams_fp64_peak(void* cuda_stream, double* h_tinstr) {
+  if (!h_tinstr) return fail(nullptr, STREAMS_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "streams_fp64_peak: no CUDA device");
+  double* d_out = nullptr;
+  cudaEvent_t e0, e1;
+  if ((e = cudaMalloc(&d_out, sizeof(double))) != cudaSuccess) return cuda_fail(nullptr, e, "cudaMalloc");
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int grid = 2 * sms, iters = 4096;
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {                 // first pass warms up; best of the next three
+    cudaEventRecord(e0, st);
+    k_fp64_peak<<<grid, 1024, 0, st>>>(d_out, iters, 0.999999, 1e-9);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double n = (double)grid * 1024.0 * iters * 64.0;
+    if (rep > 0 && ms > 0.f) best = std::max(best, n / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "k_fp64_peak");
+  *h_tinstr = best;
+  return STREAMS_OK;
+}
+
 void streams_destroy(streams_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->st);
