@@ -62,6 +62,7 @@ def bytes_per_point_per_launch(params) -> int:
 # the ghost planes of a chunk, cross-checked against ncu's executed DFMA/DADD/DMUL counts)
 DP_INSTR_RHS, DP_FLOP_RHS = 552, 826          # residual only (streams_rhs; unfused fallback)
 DP_INSTR_STAGE, DP_FLOP_STAGE = 111, 170      # + the fused RK stage: Eq. 11, primitives of the new state incl. mu(T)
+DP_INSTR_MU, DP_FLOP_MU = 56, 90              # of which mu(T) = exp(0.76 log t); with lazy forcing k_force_fix evaluates it
 FP64_LANES_PER_SM, N_SM = 64, 148             # B200: fp64 lane-instructions per SM per clock (ncu peak_sustained = 64)
 
 
@@ -259,8 +260,9 @@ def run_ours(args, rank, world, local_rank):
         if not args.no_cpu:
             r = oracle_sample(wl, 1, planes=args.ref_planes)
             cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
-        dp_instr = DP_INSTR_RHS + (DP_INSTR_STAGE if fused else 0)
-        dp_flop = DP_FLOP_RHS + (DP_FLOP_STAGE if fused else 0)
+        lazy = fused and bool(wl.params["forcing"])
+        dp_instr = DP_INSTR_RHS + (DP_INSTR_STAGE if fused else 0) - (DP_INSTR_MU if lazy else 0)
+        dp_flop = DP_FLOP_RHS + (DP_FLOP_STAGE if fused else 0) - (DP_FLOP_MU if lazy else 0)
         sm_clk = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
         alu_peak = 2.0 * FP64_LANES_PER_SM * N_SM * sm_clk / 1e12           # TFLOP/s, FMA = 2 flop
         alu_achieved = dp_flop * npts / (rhs_avg_ms * 1e-3) / 1e12

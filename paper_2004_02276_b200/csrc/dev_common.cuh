@@ -88,6 +88,7 @@ __device__ __forceinline__ void prim2cons(const DevP& P, const Prim& q, double w
 // increments of the primitives (exactly the same map; dW = 0 leaves the node bit-identical):
 //   rho' = rho + dW0,  u' = u + (dW_u - u dW0)/rho',  E' = E + (dW_E - E dW0)/rho',
 //   c_v T' = c_v T + (E' - E) - (|u'|^2 - |u|^2)/2
+template <bool WITH_MU = true>
 __device__ __forceinline__ void advance_prim(const DevP& P, Prim& q, const double dW[5]) {
   const double rn = q.rho + dW[0];
   const double ir = 1.0 / rn;
@@ -98,7 +99,7 @@ __device__ __forceinline__ void advance_prim(const DevP& P, Prim& q, const doubl
   const double dke = 0.5 * (du * (un + q.u) + dv * (vn + q.v) + dw * (wn + q.w));
   q.T = fma(dE - dke, P.inv_cv, q.T);
   q.rho = rn; q.u = un; q.v = vn; q.w = wn;
-  q.mu = visc_mu(P, q.T);
+  if (WITH_MU) q.mu = visc_mu(P, q.T);
   q.H = fma(P.cp, q.T, 0.5 * fma(un, un, fma(vn, vn, wn * wn)));
 }
 // S1: Dirichlet override of a WALL_ISO_NODE wall node after every stage (rho evolves by the scheme)

@@ -72,6 +72,9 @@ struct RhsArgs {
                           // previous R WITHOUT its forcing terms; they are added here as f_prev (e_rhou + u_prev e_rhoE),
                           // u_prev = the velocity still sitting in q_out (the previous stage's input state)
   double alpha, beta;
+  int lazy;               // FUSED: 1 = lazy forcing: k_force_fix rewrites u, T, mu, H of every node afterwards, so mu(T) is
+                          // not evaluated here (the power law is the longest dependency chain of the epilogue)
+  int write_S;            // FUSED: 0 in the last stage (alpha of the next stage is 0: R is never read)
   double* partial;        // per-CTA partial sums of R_rhou * vol (forcing), may be NULL
   int lz;                 // planes per CTA
   int use_tma;            // 1: tile by TMA box copies (tensor map over q); 0: every slot by index (odd nx)
@@ -358,6 +361,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
   const bool edge = !use_tma || i0 < HALO || i0 + TX + HALO > P.nx || j0 < HALO || j0 + TY + HALO > P.ny;
   const int nplanes = k1 + 3 - (k0 - 3);
+  const bool zfirst = (tid & (NT / 2)) != 0;             // warps 4..7 (the second warp of each scheduler)
 
   if (tid == 0) {
     *pcount = 0;
@@ -461,6 +465,37 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     asm volatile("" : "+r"(tl));                         // hoisted out of the loop (and then spilled) instead of recomputed
     const int li = tl & (TX - 1), lj = tl / TX, loc = (lj + HALO) * PITCH + li + XH;
     const double* own3 = oring + b3 * NF * NPT + tl;     // own node of plane s+3
+    // ---- z, from the register windows (no shared tile, no barrier): the upper half of the warps does it FIRST, the
+    // lower half after arriving at the barrier, so that the two warps of a scheduler are in different phases
+    // (fp64-dense z against the shared-memory-heavy x, y)
+    NodeAcc N;
+    auto zdir = [&]() {
+      Nb c;
+      c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
+      DirAcc Z;
+      acc_zero(Z);
+#pragma unroll
+      for (int l = 1; l <= 3; ++l) {
+        Nb p, m;
+        if (l < 3) {
+          p.rho = rw[3 + l]; p.u = uw[3 + l]; p.v = vw[3 + l]; p.w = ww[3 + l]; p.T = Tw[3 + l]; p.mu = mw[3 + l]; p.H = Hw[3 + l];
+        } else {
+          p.rho = own3[F_RHO * NPT]; p.u = own3[F_U * NPT]; p.v = own3[F_V * NPT]; p.w = own3[F_W * NPT];
+          p.T = own3[F_T * NPT]; p.mu = own3[F_MU * NPT]; p.H = own3[F_H * NPT];
+        }
+        m.rho = rw[3 - l]; m.u = uw[3 - l]; m.v = vw[3 - l]; m.w = ww[3 - l]; m.T = Tw[3 - l]; m.mu = mw[3 - l]; m.H = Hw[3 - l];
+        dir_accum<2>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Z);
+      }
+      double f[5];
+      conv_from_acc<2>(c, Z, f);
+      dir_fold<2>(P, c, Z, f, zi[s - k0], zg[s - k0], N);
+    };
+    if (active && full) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) N.R[v] = 0.0;
+      N.Va[0] = N.Va[1] = N.Va[2] = 0.0; N.LT = 0.0; N.heat = 0.0;
+      if (zfirst) zdir();
+    }
     if (use_tma) mbar_wait(bar0 + 8 * buf, phase);
     if (edge && it + 1 < nplanes) {
       // ghost slots of the NEXT plane's tile: written before this step's barrier, read after it
@@ -480,7 +515,6 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
       sgX[(jo + HALO) * TX + col] = d1_tile(P, t + F_U * TILE, (jo + HALO) * PITCH + col + XH, 1);
     }
 
-    NodeAcc N;
     if (!active || !full) {
       // ghost planes of the chunk, and tile nodes beyond the grid (their staging entries are the
       // neighbours' ghost columns / rows): in-plane first derivatives only
@@ -500,9 +534,6 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
       {
         Nb c;
         c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) N.R[v] = 0.0;
-        N.Va[0] = N.Va[1] = N.Va[2] = 0.0; N.LT = 0.0; N.heat = 0.0;
         // ---- x ----
         {
           DirAcc X;
@@ -551,30 +582,10 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     __syncwarp();
     if ((tl & 31) == 0) mbar_arrive(sbar);
 
-    if (active && full) {
-      // ---- z, from the register windows ----
-      Nb c;
-      c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
-      DirAcc Z;
-      acc_zero(Z);
-#pragma unroll
-      for (int l = 1; l <= 3; ++l) {
-        Nb p, m;
-        if (l < 3) {
-          p.rho = rw[3 + l]; p.u = uw[3 + l]; p.v = vw[3 + l]; p.w = ww[3 + l]; p.T = Tw[3 + l]; p.mu = mw[3 + l]; p.H = Hw[3 + l];
-        } else {
-          p.rho = own3[F_RHO * NPT]; p.u = own3[F_U * NPT]; p.v = own3[F_V * NPT]; p.w = own3[F_W * NPT];
-          p.T = own3[F_T * NPT]; p.mu = own3[F_MU * NPT]; p.H = own3[F_H * NPT];
-        }
-        m.rho = rw[3 - l]; m.u = uw[3 - l]; m.v = vw[3 - l]; m.w = ww[3 - l]; m.T = Tw[3 - l]; m.mu = mw[3 - l]; m.H = Hw[3 - l];
-        dir_accum<2>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Z);
-      }
-      double f[5];
-      conv_from_acc<2>(c, Z, f);
-      dir_fold<2>(P, c, Z, f, zi[s - k0], zg[s - k0], N);
-    }
+    if (!zfirst && active && full) zdir();
     // ---- second half of the barrier: the staging rows of this plane are complete ----
     mbar_wait(sbar, (unsigned)(it & 1));
+    if (FUSED) cp_async_wait<0>();                       // R_prev / u_prev of plane s-3 (requested at the top of the step)
     // every thread is past its reads of this plane's tile: the buffer takes plane s+2
     if (use_tma && tl == 0 && it + 2 < nplanes) {
       const int b2 = buf;                                // (it + 2) % NBUF
@@ -618,7 +629,6 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
       } else {
         double dW[5];
         const double dt = scal[0], fprev = scal[1];
-        cp_async_wait<0>();                              // R_prev / u_prev of this plane (requested at the top of the step)
         const double* pv = spring + tl;
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
@@ -626,14 +636,16 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
           if (v == 1) sp += fprev;
           if (v == 4 && A.f_prev && A.alpha != 0.0) sp = fma(fprev, pv[5 * NPT], sp);
           dW[v] = dt * (A.alpha * sp + A.beta * R[v]);
-          A.S_out[o + v * P.N] = R[v];
+          if (A.write_S) A.S_out[o + v * P.N] = R[v];
         }
         Prim qn; qn.rho = rw[0]; qn.u = uw[0]; qn.v = vw[0]; qn.w = ww[0]; qn.T = Tw[0]; qn.mu = mw[0]; qn.H = 0.0;
-        advance_prim(P, qn, dW);
-        if (gj == 0 && P.bc[2] == BC_WALL_NODE) wall_node_override(P, P.Twall[0], P.mu_wall[0], qn);
-        if (gj == P.ny - 1 && P.bc[3] == BC_WALL_NODE) wall_node_override(P, P.Twall[1], P.mu_wall[1], qn);
+        bool store_mu = !A.lazy;
+        if (A.lazy) advance_prim<false>(P, qn, dW); else advance_prim<true>(P, qn, dW);
+        if (gj == 0 && P.bc[2] == BC_WALL_NODE) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
+        if (gj == P.ny - 1 && P.bc[3] == BC_WALL_NODE) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
         A.q_out[o] = qn.rho; A.q_out[o + P.N] = qn.u; A.q_out[o + 2 * P.N] = qn.v; A.q_out[o + 3 * P.N] = qn.w;
-        A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 5 * P.N] = qn.mu; A.q_out[o + 6 * P.N] = qn.H;
+        A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 6 * P.N] = qn.H;
+        if (store_mu) A.q_out[o + 5 * P.N] = qn.mu;
       }
     }
     if (active && full) {

@@ -562,6 +562,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         double* wn = c->qbuf[c->cur ^ 1];
         A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
         A.f_prev = l > 0 ? &c->sc->force : nullptr;
+        A.lazy = 1; A.write_S = l < 2 ? 1 : 0;
         if ((rc = launch_rhs(c, true, A))) return rc;
         if ((rc = force_from_partials(c, nullptr, true))) return rc;
         k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l]);
@@ -585,7 +586,7 @@ int streams_step(streams_ctx* c, int nsteps) {
       } else {
         // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
         double* wn = c->qbuf[c->cur ^ 1];
-        A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0];
+        A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
         if ((rc = launch_rhs(c, true, A))) return rc;
         if (c->p.weno_enable) {
           k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->S[0], wn, beta[l]);
