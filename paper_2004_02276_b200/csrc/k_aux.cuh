@@ -16,6 +16,7 @@ struct DevScal {
   unsigned long long weno_if[3];
   unsigned int list_count;
   unsigned int pad;
+  double dt_next;       // S10 evaluated on the state at the end of a step (fused into the last k_force_fix)
 };
 
 // ---- S3: conservative w[5][N] -> primitives Q[NQ][N]  (streams_set_state) ----
@@ -71,27 +72,66 @@ __global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, d
 
 // ---- lazy forcing (S9 with Eq. 11): the fused k_rhs<true> advanced the state WITHOUT this stage's body force (f is
 // only known once the whole R has been summed); this adds dt beta f (e_rhou + u e_rhoE), u = the velocity of the
-// stage's input state `Qin`, to the new state `Q` (rho, v, w are not touched).  Same map as advance_prim.
+// stage's input state `Qin`, to the new state `Q` (rho, v, w are not touched) and evaluates mu(T) of the new state.
+// Same map as advance_prim.  One CTA walks grid rows (j,k); `speed` != NULL (last stage): per-CTA maxima of
+// (|u_d| + c) / h_d of the finished state (S10) go to speed[3][gridDim.x], so the next step needs no extra pass.
+constexpr int FIXU = 4;
 __global__ void __launch_bounds__(RT) k_force_fix(const __grid_constant__ DevP P, double* __restrict__ Q, const double* __restrict__ Qin,
-                                                  const DevScal* __restrict__ sc, double beta) {
+                                                  const DevScal* __restrict__ sc, double beta, double* __restrict__ speed) {
+  __shared__ double sh[RT / 32];
   const double c = sc->dt * beta * sc->force;
   const bool wn0 = P.bc[2] == BC_WALL_NODE, wn1 = P.bc[3] == BC_WALL_NODE;
-  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    if (wn0 || wn1) {
-      const int j = (int)((o / P.nx) % P.ny);
-      if ((wn0 && j == 0) || (wn1 && j == P.ny - 1)) continue;      // Dirichlet wall node: already overridden
+  const int nrows = P.ny * P.nz;
+  double m[3] = {0.0, 0.0, 0.0};
+  for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+    const int j = row % P.ny, k = row / P.ny;
+    const bool wallrow = (wn0 && j == 0) || (wn1 && j == P.ny - 1);      // Dirichlet wall nodes: already overridden
+    const double ihy = P.ih[1][j], ihz = P.ih[2][k];
+    const size_t r0 = (size_t)row * P.nx;
+    for (int ib = threadIdx.x; ib < P.nx; ib += FIXU * RT) {
+      // FIXU nodes per thread, all loads first (memory-level parallelism: the kernel is HBM-bound)
+      double rho[FIXU], u[FIXU], T[FIXU], H[FIXU], ul[FIXU], vv[FIXU], ww[FIXU];
+#pragma unroll
+      for (int e = 0; e < FIXU; ++e) {
+        const int i = ib + e * RT;
+        if (i < P.nx) {
+          const size_t o = r0 + i;
+          u[e] = Q[o + P.N]; T[e] = Q[o + 4 * P.N];
+          if (!wallrow) { rho[e] = Q[o]; H[e] = Q[o + 6 * P.N]; ul[e] = Qin[o + P.N]; }
+          if (speed) { vv[e] = Q[o + 2 * P.N]; ww[e] = Q[o + 3 * P.N]; }
+        }
+      }
+#pragma unroll
+      for (int e = 0; e < FIXU; ++e) {
+        const int i = ib + e * RT;
+        if (i < P.nx) {
+          const size_t o = r0 + i;
+          double un = u[e], Tn = T[e];
+          if (!wallrow) {
+            const double ir = 1.0 / rho[e];
+            const double du = c * ir, dE = (c * ul[e]) * ir;
+            un = u[e] + du;
+            const double dke = 0.5 * (du * (un + u[e]));
+            const double dT = (dE - dke) * P.inv_cv;
+            Tn = T[e] + dT;
+            Q[o + P.N] = un; Q[o + 4 * P.N] = Tn; Q[o + 5 * P.N] = visc_mu(P, Tn);
+            Q[o + 6 * P.N] = H[e] + fma(P.cp, dT, dke);
+          }
+          if (speed) {
+            const double cs = sqrt(P.gam * P.Rgas * Tn);
+            m[0] = fmax(m[0], (fabs(un) + cs) * P.ih[0][i]);
+            m[1] = fmax(m[1], (fabs(vv[e]) + cs) * ihy);
+            m[2] = fmax(m[2], (fabs(ww[e]) + cs) * ihz);
+          }
+        }
+      }
     }
-    const double rho = Q[o], u = Q[o + P.N], T = Q[o + 4 * P.N], H = Q[o + 6 * P.N];
-    const double ul = Qin[o + P.N];
-    const double ir = 1.0 / rho;
-    const double du = c * ir, dE = (c * ul) * ir;
-    const double un = u + du;
-    const double dke = 0.5 * (du * (un + u));
-    const double dT = (dE - dke) * P.inv_cv;
-    const double Tn = T + dT;
-    Q[o + P.N] = un; Q[o + 4 * P.N] = Tn; Q[o + 5 * P.N] = visc_mu(P, Tn);
-    Q[o + 6 * P.N] = H + fma(P.cp, dT, dke);
   }
+  if (speed)
+    for (int d = 0; d < 3; ++d) {
+      const double t = block_max<RT>(m[d], sh, threadIdx.x);
+      if (threadIdx.x == 0) speed[d * gridDim.x + blockIdx.x] = t;
+    }
 }
 
 // R_rhou += f, R_rhoE += f u  (streams_rhs with forcing)
@@ -150,9 +190,11 @@ __global__ void __launch_bounds__(RT) k_dt_final(const double* __restrict__ part
     const double t = block_max<RT>(m, sh, threadIdx.x);
     if (threadIdx.x == 0) { mm = fmax(mm, t); if (speeds_out) speeds_out[d] = t; }
   }
-  if (threadIdx.x == 0 && set_dt) sc->dt = dt_fixed > 0.0 ? dt_fixed : cfl / mm;
+  if (threadIdx.x == 0 && set_dt == 1) sc->dt = dt_fixed > 0.0 ? dt_fixed : cfl / mm;
+  if (threadIdx.x == 0 && set_dt == 2) sc->dt_next = dt_fixed > 0.0 ? dt_fixed : cfl / mm;
 }
 __global__ void k_advance_time(DevScal* sc) { sc->time += sc->dt; }
+__global__ void k_take_dt(DevScal* sc) { sc->dt = sc->dt_next; }
 
 // ---- diagnostics: per-block partials, reduced on the host by streams_diagnostics ----
 constexpr int NDIAG = 12;   // mass, mx, my, mz, E, ke, vol | min rho, min p, max Mach | nonfinite | spare

@@ -45,6 +45,7 @@ struct streams_ctx {
   long long launches;
   dim3 rhs_grid;
   int lz;
+  int dt_ready;                        // sc->dt_next holds the CFL step of the current state (last k_force_fix of a step)
   CUtensorMap tmap[2];           // TMA descriptors of qbuf[0], qbuf[1] as 4-D tensors (x, y, z, field)
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
   int prof_on, prof_n;
@@ -434,7 +435,7 @@ static int after_set_state(streams_ctx* c, const double* d_w) {
   CK(cudaMemsetAsync(&c->sc->force, 0, sizeof(double), c->st));
   CK(cudaMemsetAsync(&c->sc->time, 0, sizeof(double), c->st));
   if (!(c->p.dt_fixed > 0.0)) CK(cudaMemsetAsync(&c->sc->dt, 0, sizeof(double), c->st));
-  c->has_state = 1; c->step = 0; c->scur = 0;
+  c->has_state = 1; c->step = 0; c->scur = 0; c->dt_ready = 0;
   return STREAMS_OK;
 }
 
@@ -544,7 +545,11 @@ int streams_step(streams_ctx* c, int nsteps) {
   const int rg = rgrid_for(c->P.N);
   int rc;
   for (int s = 0; s < nsteps; ++s) {
-    if (!(c->p.dt_fixed > 0.0)) {
+    if (!(c->p.dt_fixed > 0.0) && c->dt_ready) {
+      k_take_dt<<<1, 1, 0, c->st>>>(c->sc);
+      LAUNCH_CHECK("k_take_dt");
+      c->dt_ready = 0;
+    } else if (!(c->p.dt_fixed > 0.0)) {
       k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->partial);
       LAUNCH_CHECK("k_speed_partial");
       k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 1);
@@ -565,8 +570,14 @@ int streams_step(streams_ctx* c, int nsteps) {
         A.lazy = 1; A.write_S = l < 2 ? 1 : 0;
         if ((rc = launch_rhs(c, true, A))) return rc;
         if ((rc = force_from_partials(c, nullptr, true))) return rc;
-        k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l]);
+        const bool want_dt = l == 2 && !(c->p.dt_fixed > 0.0);
+        k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l], want_dt ? c->partial : nullptr);
         LAUNCH_CHECK("k_force_fix");
+        if (want_dt) {
+          k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 2);
+          LAUNCH_CHECK("k_dt_final");
+          c->dt_ready = 1;
+        }
         c->cur ^= 1;
       } else if (c->p.forcing) {
         // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
