@@ -325,9 +325,12 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
 }
 
 
-template <bool FUSED>
-__global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
-  extern __shared__ __align__(128) double sm[];
+// The whole kernel body.  PLAIN = true is the instantiation for tiles that lie fully inside the grid and hold no
+// special node (no staggered-wall row, no Dirichlet wall row, no characteristic outflow column), with TMA and the
+// viscous terms on: every such test folds at compile time and no out-of-line call remains in the plane loop, which
+// frees ~30 registers for the scheduler.  Ghost slots (periodic wrap, reflection, ...) are handled in both.
+template <bool FUSED, bool PLAIN>
+__device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const CUtensorMap& tmap, double* sm) {
   double* tiles = sm;
   double* stg = tiles + SM_TILES;
   double* gring = stg + 2 * SM_STG1;
@@ -354,10 +357,10 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const int gi = i0 + ti, gj = j0 + tj;
   const int k0 = blockIdx.z * A.lz;
   const int k1 = min(k0 + A.lz, P.nz);
-  const bool active = gi < P.nx && gj < P.ny;
+  const bool active = PLAIN || (gi < P.nx && gj < P.ny);
   const int oc = (tj + HALO) * PITCH + ti + XH;                               // own tile offset
   const int own_off = gj * P.nx + gi;
-  const bool use_tma = A.use_tma != 0;
+  const bool use_tma = PLAIN || A.use_tma != 0;
   // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
   const bool edge = !use_tma || i0 < HALO || i0 + TX + HALO > P.nx || j0 < HALO || j0 + TY + HALO > P.ny;
   const int nplanes = k1 + 3 - (k0 - 3);
@@ -546,7 +549,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
           sgX[(lj + HALO) * TX + li] = X.du;                                 // D_x u, for d_y(d_x u) of the neighbours
           double f[5];
           conv_from_acc<0>(c, X, f);
-          if (gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) {
+          if (!PLAIN && gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) {
             const F5 r = outflow_x(P, t, loc);
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
@@ -567,7 +570,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
           conv_from_acc<1>(c, Y, f);
           const bool wall_lo = gj == 0 && P.bc[2] == BC_WALL_STAG;
           const bool wall_hi = gj == P.ny - 1 && P.bc[3] == BC_WALL_STAG;
-          if (wall_lo || wall_hi) {
+          if (!PLAIN && (wall_lo || wall_hi)) {
             const F5 r = wall_y(P, t, loc, wall_lo, wall_hi);
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
@@ -602,7 +605,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
 #pragma unroll
         for (int v = 0; v < 5; ++v) R[v] = rr[v * NPT];
       }
-      if (P.viscous) {
+      if (PLAIN || P.viscous) {
         // ring slot of plane p+l is (slot7 - 3 + l) mod 7
         double dz[3] = {0.0, 0.0, 0.0};
 #pragma unroll
@@ -641,15 +644,15 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
         Prim qn; qn.rho = rw[0]; qn.u = uw[0]; qn.v = vw[0]; qn.w = ww[0]; qn.T = Tw[0]; qn.mu = mw[0]; qn.H = 0.0;
         bool store_mu = !A.lazy;
         if (A.lazy) advance_prim<false>(P, qn, dW); else advance_prim<true>(P, qn, dW);
-        if (gj == 0 && P.bc[2] == BC_WALL_NODE) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
-        if (gj == P.ny - 1 && P.bc[3] == BC_WALL_NODE) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
+        if (!PLAIN && gj == 0 && P.bc[2] == BC_WALL_NODE) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
+        if (!PLAIN && gj == P.ny - 1 && P.bc[3] == BC_WALL_NODE) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
         A.q_out[o] = qn.rho; A.q_out[o + P.N] = qn.u; A.q_out[o + 2 * P.N] = qn.v; A.q_out[o + 3 * P.N] = qn.w;
         A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 6 * P.N] = qn.H;
         if (store_mu) A.q_out[o + 5 * P.N] = qn.mu;
       }
     }
     if (active && full) {
-      if (P.viscous) {
+      if (PLAIN || P.viscous) {
         // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
         const int sy = lj * PITCH + li + XH, sx = (lj + HALO) * TX + li;
         double mxy = P.c.a[0] * (sgY[sy + 1] - sgY[sy - 1]);
@@ -686,6 +689,18 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
     const double tot = block_sum<NT>(fsum * hxy, red, tid);
     if (tid == 0) A.partial[(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = tot;
   }
+}
+
+template <bool FUSED>
+__global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
+  extern __shared__ __align__(128) double sm[];
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const bool inside = i0 + TX <= P.nx && j0 + TY <= P.ny;
+  const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
+  const bool wall_lo = (P.bc[2] == BC_WALL_STAG || P.bc[2] == BC_WALL_NODE) && j0 == 0;
+  const bool wall_hi = (P.bc[3] == BC_WALL_STAG || P.bc[3] == BC_WALL_NODE) && j0 + TY >= P.ny;
+  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<FUSED, true>(P, A, tmap, sm);
+  else rhs_body<FUSED, false>(P, A, tmap, sm);
 }
 
 }  // namespace streams
