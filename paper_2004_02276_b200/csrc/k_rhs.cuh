@@ -364,7 +364,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
   const bool edge = !use_tma || i0 < HALO || i0 + TX + HALO > P.nx || j0 < HALO || j0 + TY + HALO > P.ny;
   const int nplanes = k1 + 3 - (k0 - 3);
-  const bool zfirst = (tid & (NT / 2)) != 0;             // warps 4..7 (the second warp of each scheduler)
+  constexpr bool zfirst = false;                         // (phase stagger between warp halves: measured +1 %, costs a second copy of the z block)
 
   if (tid == 0) {
     *pcount = 0;
