@@ -211,6 +211,28 @@ __device__ __forceinline__ void fetch_prim(const DevP& P, const double* __restri
   load_src_raw(P, Q, s, map_z(P, k), q);
   apply_reflect(P, s, q);
 }
+// rho, u, v, w, T only (WENO stencils: p, H and c are derived; mu is not needed, so a reflected ghost pays no power law)
+__device__ __forceinline__ void fetch_prim5(const DevP& P, const double* __restrict__ Q, int i, int j, int k, Prim& q) {
+  const Src s = resolve_xy(P, i, j);
+  const int kk = map_z(P, k), kd = s.kind & 7;
+  if (kd == SRC_FIELD) {
+    const size_t o = (size_t)kk * P.nxy + s.off;
+    q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.N); q.v = __ldg(Q + o + 2 * P.N); q.w = __ldg(Q + o + 3 * P.N); q.T = __ldg(Q + o + 4 * P.N);
+  } else if (kd == SRC_INFLOW) {
+    const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
+    q.rho = P.inflow[o]; q.u = P.inflow[o + st]; q.v = P.inflow[o + 2 * st]; q.w = P.inflow[o + 3 * st]; q.T = P.inflow[o + 4 * st];
+  } else {
+    const double* c = kd == SRC_POST ? P.post : P.fs;
+    q.rho = c[0]; q.u = c[1]; q.v = c[2]; q.w = c[3]; q.T = c[4];
+  }
+  const int r = s.kind >> 4;
+  if (r) {                                   // S1 isothermal no-slip reflection (see reflect())
+    const double Tg = 2.0 * P.Twall[r - 1] - q.T;
+    q.rho = (q.rho * q.T) / Tg;
+    q.u = -q.u; q.v = -q.v; q.w = -q.w; q.T = Tg;
+  }
+  q.mu = 0.0; q.H = 0.0;
+}
 // velocities only (sensor)
 __device__ __forceinline__ void fetch_vel(const DevP& P, const double* __restrict__ Q, int i, int j, int k, double& u, double& v, double& w) {
   const Src s = resolve_xy(P, i, j);

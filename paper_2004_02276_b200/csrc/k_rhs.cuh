@@ -75,6 +75,8 @@ struct RhsArgs {
   int lazy;               // FUSED: 1 = lazy forcing: k_force_fix rewrites u, T, mu, H of every node afterwards, so mu(T) is
                           // not evaluated here (the power law is the longest dependency chain of the epilogue)
   int write_S;            // FUSED: 0 in the last stage (alpha of the next stage is 0: R is never read)
+  unsigned char* nflag;   // hybrid switch on: node flags theta > theta_th of Eq. 8 (a3), a by-product of the velocity
+                          // gradients; [N] bytes, NULL when the WENO switch is off
   double* partial;        // per-CTA partial sums of R_rhou * vol (forcing), may be NULL
   int lz;                 // planes per CTA
   int use_tma;            // 1: tile by TMA box copies (tensor map over q); 0: every slot by index (odd nx)
@@ -652,6 +654,14 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       }
     }
     if (active && full) {
+      if (A.nflag) {
+        // S4 / Eq. 8: same expression, same order as k_sensor (the flags must agree bit for bit)
+        const double* G = N.G;
+        const double div = G[0] + G[4] + G[8];
+        const double ox = G[7] - G[5], oy = G[2] - G[6], oz = G[3] - G[1];
+        const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
+        A.nflag[(size_t)s * P.nxy + own_off] = th > P.th_thr ? 1 : 0;
+      }
       if (PLAIN || P.viscous) {
         // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
         const int sy = lj * PITCH + li + XH, sx = (lj + HALO) * TX + li;

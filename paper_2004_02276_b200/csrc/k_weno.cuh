@@ -70,23 +70,38 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
                                                   unsigned int* __restrict__ list, unsigned char* __restrict__ lmask,
                                                   unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
   unsigned long long cnt[3] = {0, 0, 0};
-  for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+  // every lane runs the same number of iterations (the ballot below needs the whole warp); lanes past the end idle
+  const long long nround = (P.N + (long long)gridDim.x * RT - 1) / ((long long)gridDim.x * RT);
+  for (long long it = 0; it < nround; ++it) {
+    const long long o = (it * gridDim.x + blockIdx.x) * (long long)RT + threadIdx.x;
+    const bool in = o < P.N;
+    const int i = in ? (int)(o % P.nx) : 0, j = in ? (int)((o / P.nx) % P.ny) : 0, k = in ? (int)(o / P.nxy) : 0;
     const int id[3] = {i, j, k};
     int mask = 0;
+    if (in) {
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      const int lo = iface_flag(P, nflag, d, i, j, k, id[d] - 1);
-      const int hi = iface_flag(P, nflag, d, i, j, k, id[d]);
-      mask |= (lo << (2 * d)) | (hi << (2 * d + 1));
-      cnt[d] += hi;
-      if (id[d] == 0 && P.bc[2 * d] != BC_PERIODIC) cnt[d] += lo;
-      if (iflags_out) iflags_out[d * P.N + o] = (unsigned char)hi;
+      for (int d = 0; d < 3; ++d) {
+        const int lo = iface_flag(P, nflag, d, i, j, k, id[d] - 1);
+        const int hi = iface_flag(P, nflag, d, i, j, k, id[d]);
+        mask |= (lo << (2 * d)) | (hi << (2 * d + 1));
+        cnt[d] += hi;
+        if (id[d] == 0 && P.bc[2 * d] != BC_PERIODIC) cnt[d] += lo;
+        if (iflags_out) iflags_out[d * P.N + o] = (unsigned char)hi;
+      }
     }
-    if (mask && list) {
-      const unsigned int pos = atomicAdd(&sc->list_count, 1u);
-      list[pos] = (unsigned int)o;
-      lmask[pos] = (unsigned char)mask;
+    // warp-aggregated append: the listed nodes of a warp take consecutive slots in lane (= x) order, so that
+    // k_weno_apply reads its stencils coalesced
+    const unsigned int bal = __ballot_sync(0xffffffffu, mask != 0 && list != nullptr);
+    if (bal) {
+      const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+      unsigned int base = 0;
+      if (lane == leader) base = atomicAdd(&sc->list_count, (unsigned int)__popc(bal));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (mask && list) {
+        const unsigned int pos = base + __popc(bal & ((1u << lane) - 1u));
+        list[pos] = (unsigned int)o;
+        lmask[pos] = (unsigned char)mask;
+      }
     }
   }
 #pragma unroll
@@ -121,7 +136,7 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
   for (int n = 0; n < 6; ++n) {
     const int off = n - 2;
     Prim q;
-    fetch_prim(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0), q);
+    fetch_prim5(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0), q);
     rho[n] = q.rho; vel[n][0] = q.u; vel[n][1] = q.v; vel[n][2] = q.w;
     derive_pH(P, q.rho, q.u, q.v, q.w, q.T, pp[n], Hh[n]);
     cs[n] = sqrt(P.gam * P.Rgas * q.T);

@@ -480,9 +480,18 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
   return STREAMS_OK;
 }
 
+// list of nodes with flagged interfaces from the node flags k_rhs has just written (a3)
+static int run_list(streams_ctx* c) {
+  CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
+  k_weno_list<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->list, c->lmask, nullptr, c->sc);
+  LAUNCH_CHECK("k_weno_list");
+  return STREAMS_OK;
+}
+
 static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A_in) {
   RhsArgs A = A_in;
   A.use_tma = c->use_tma;
+  A.nflag = c->p.weno_enable ? c->nflag : nullptr;
   const CUtensorMap& tm = c->tmap[A.q == c->qbuf[1] ? 1 : 0];
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
@@ -511,7 +520,6 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   const double* w = c->qbuf[c->cur];
   int rc;
-  if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, true))) return rc;
   RhsArgs A;
   std::memset(&A, 0, sizeof A);
   A.q = w; A.out_rhs = d_rhs; A.lz = c->lz;
@@ -519,6 +527,7 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   A.partial = partial_ok ? c->partial : nullptr;
   if ((rc = launch_rhs(c, false, A))) return rc;
   if (c->p.weno_enable) {
+    if ((rc = run_list(c))) return rc;
     k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, d_rhs, nullptr, 0.0);
     LAUNCH_CHECK("k_weno_apply");
   }
@@ -557,7 +566,6 @@ int streams_step(streams_ctx* c, int nsteps) {
     }
     for (int l = 0; l < 3; ++l) {
       double* w = c->qbuf[c->cur];
-      if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, true))) return rc;
       RhsArgs A;
       std::memset(&A, 0, sizeof A);
       A.q = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
@@ -587,6 +595,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
         if ((rc = launch_rhs(c, false, A))) return rc;
         if (c->p.weno_enable) {
+          if ((rc = run_list(c))) return rc;
           k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, Sc, nullptr, 0.0);
           LAUNCH_CHECK("k_weno_apply");
         }
@@ -600,6 +609,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
         if ((rc = launch_rhs(c, true, A))) return rc;
         if (c->p.weno_enable) {
+          if ((rc = run_list(c))) return rc;
           k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->S[0], wn, beta[l]);
           LAUNCH_CHECK("k_weno_apply");
         }
