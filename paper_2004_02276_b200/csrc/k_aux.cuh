@@ -17,6 +17,8 @@ struct DevScal {
   unsigned int list_count;
   unsigned int pad;
   double dt_next;       // S10 evaluated on the state at the end of a step (fused into the last k_force_fix)
+  unsigned int icount[3];   // entries of the three interface lists (k_weno_list)
+  unsigned int pad2;
 };
 
 // ---- S3: conservative w[5][N] -> primitives Q[NQ][N]  (streams_set_state) ----

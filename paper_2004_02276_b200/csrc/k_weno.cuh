@@ -3,10 +3,13 @@
 // The hybrid switch is hard (A6): interface i+1/2 takes the characteristic-wise
 // Lax-Friedrichs WENO5 flux when any of its six stencil nodes has theta > theta_th, the
 // central flux otherwise.  The fused kernel evaluates the central flux
-// everywhere; here the few flagged interfaces add  dF = F_weno - F_central  to their two
-// nodes.  Work is compacted: k_weno_list appends every node with at least one flagged
-// interface, k_weno_apply runs one thread per listed node (no divergence on clean warps, no
-// floating-point atomics: each node sums its own corrections in a fixed order).
+// everywhere; here the flagged interfaces add  dF = F_weno - F_central  to their two nodes.
+// Work is compacted and done ONCE per interface: k_weno_list appends every flagged interface
+// i+1/2 (by its lower node) to the list of its direction and every node with at least one
+// flagged interface to the node list; k_weno_flux<D> runs one thread per listed interface (no
+// divergence) and leaves dF in a node-indexed scratch array; k_weno_apply runs one thread per
+// listed node and sums the corrections of its up to six interfaces in a fixed order (no
+// floating-point atomics: deterministic).
 #pragma once
 #include "dev_common.cuh"
 #include "k_aux.cuh"
@@ -65,9 +68,26 @@ __device__ __forceinline__ int iface_flag(const DevP& P, const unsigned char* __
   return any;
 }
 
+constexpr unsigned int IFACE_BELOW = 0x80000000u;      // interface-list entry: the interface BELOW the (first) node
+// offset of node (i,j,k) inside the boundary plane of direction D (scratch of the IFACE_BELOW entries)
+template <int D>
+__device__ __forceinline__ size_t plane_index(const DevP& P, int i, int j, int k) {
+  return D == 0 ? (size_t)k * P.ny + j : (D == 1 ? (size_t)k * P.nx + i : (size_t)j * P.nx + i);
+}
+template <int D>
+__device__ __forceinline__ size_t plane_size(const DevP& P) {
+  return D == 0 ? (size_t)P.ny * P.nz : (D == 1 ? (size_t)P.nx * P.nz : (size_t)P.nx * P.ny);
+}
+// boundary scratch dFb: [x: 5 * ny*nz][y: 5 * nx*nz][z: 5 * nx*ny]
+template <int D>
+__device__ __forceinline__ size_t plane_base(const DevP& P) {
+  return D == 0 ? 0 : (D == 1 ? 5 * plane_size<0>(P) : 5 * (plane_size<0>(P) + plane_size<1>(P)));
+}
+
 // list of nodes with a flagged interface; entry = node index, mask bit (2d+side), side 0 = below, 1 = above
 __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P, const unsigned char* __restrict__ nflag,
                                                   unsigned int* __restrict__ list, unsigned char* __restrict__ lmask,
+                                                  unsigned int* __restrict__ ilist /* [3][istride] or NULL */, size_t istride,
                                                   unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
   unsigned long long cnt[3] = {0, 0, 0};
   // every lane runs the same number of iterations (the ballot below needs the whole warp); lanes past the end idle
@@ -89,11 +109,30 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
         if (iflags_out) iflags_out[d * P.N + o] = (unsigned char)hi;
       }
     }
-    // warp-aggregated append: the listed nodes of a warp take consecutive slots in lane (= x) order, so that
-    // k_weno_apply reads its stencils coalesced
+    // warp-aggregated appends: the entries of a warp take consecutive slots in lane (= x) order, so that the
+    // consumers read their stencils coalesced
+    const int lane = threadIdx.x & 31;
+    if (ilist) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const bool hi = (mask >> (2 * d + 1)) & 1;
+        const unsigned int bd = __ballot_sync(0xffffffffu, hi);
+        if (bd) {
+          const int leader = __ffs(bd) - 1;
+          unsigned int base = 0;
+          if (lane == leader) base = atomicAdd(&sc->icount[d], (unsigned int)__popc(bd));
+          base = __shfl_sync(0xffffffffu, base, leader);
+          if (hi) ilist[d * istride + base + __popc(bd & ((1u << lane) - 1u))] = (unsigned int)o;
+        }
+        // the interface between the ghost node and the first node of a non-periodic direction has no lower node:
+        // entry = first node | IFACE_BELOW (rare: one plane per direction; istride = N + the largest plane)
+        const bool lob = in && id[d] == 0 && P.bc[2 * d] != BC_PERIODIC && ((mask >> (2 * d)) & 1);
+        if (__any_sync(0xffffffffu, lob) && lob) ilist[d * istride + atomicAdd(&sc->icount[d], 1u)] = (unsigned int)o | IFACE_BELOW;
+      }
+    }
     const unsigned int bal = __ballot_sync(0xffffffffu, mask != 0 && list != nullptr);
     if (bal) {
-      const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+      const int leader = __ffs(bal) - 1;
       unsigned int base = 0;
       if (lane == leader) base = atomicAdd(&sc->list_count, (unsigned int)__popc(bal));
       base = __shfl_sync(0xffffffffu, base, leader);
@@ -216,11 +255,55 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
   for (int v = 0; v < 5; ++v) dF[v] = Fw[v] - Fc[v];
 }
 
+// one thread per listed interface of direction D: dF of the interface above node o -> dFbuf[D][v][o]
+// (IFACE_BELOW entries: the interface below the first node -> dFb, the boundary-plane scratch)
+template <int D>
+__global__ void __launch_bounds__(128) k_weno_flux(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ ilist,
+                                                   size_t istride, const DevScal* __restrict__ sc, double* __restrict__ dFbuf, double* __restrict__ dFb) {
+  const unsigned int n = sc->icount[D];
+  const unsigned int* li = ilist + D * istride;
+  double* out = dFbuf + (size_t)D * 5 * P.N;
+  for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+    const unsigned int en = li[e];
+    const bool below = (en & IFACE_BELOW) != 0;
+    const long long o = en & ~IFACE_BELOW;
+    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    double dF[5];
+    weno_delta<D>(P, w, i - (below && D == 0), j - (below && D == 1), k - (below && D == 2), dF);
+    if (below) {
+      double* ob = dFb + plane_base<D>(P) + plane_index<D>(P, i, j, k);
+#pragma unroll
+      for (int v = 0; v < 5; ++v) ob[v * plane_size<D>(P)] = dF[v];
+    } else {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) out[o + v * P.N] = dF[v];
+    }
+  }
+}
+
+// dF of the interface BELOW node (i,j,k) along D: the scratch entry of the lower neighbour, or of the boundary plane
+template <int D>
+__device__ __forceinline__ void dF_below(const DevP& P, const double* __restrict__ dFbuf, const double* __restrict__ dFb, int i, int j, int k, double dF[5]) {
+  const int id = D == 0 ? i : (D == 1 ? j : k), n = D == 0 ? P.nx : (D == 1 ? P.ny : P.nz);
+  if (id == 0 && P.bc[2 * D] != BC_PERIODIC) {
+    const double* ib = dFb + plane_base<D>(P) + plane_index<D>(P, i, j, k);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dF[v] = ib[v * plane_size<D>(P)];
+    return;
+  }
+  const int im = id == 0 ? n - 1 : id - 1;
+  const size_t o = ((size_t)(D == 2 ? im : k) * P.ny + (D == 1 ? im : j)) * P.nx + (D == 0 ? im : i);
+  const double* in = dFbuf + (size_t)D * 5 * P.N;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) dF[v] = in[o + v * P.N];
+}
+
 // one thread per listed node: R += dR, and (if q_new) the node of the already advanced state takes the
 // conservative increment dt beta dR  (Eq. 11 is linear in R)
-__global__ void __launch_bounds__(128) k_weno_apply(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
-                                                    const unsigned char* __restrict__ lmask, const DevScal* __restrict__ sc,
-                                                    double* __restrict__ R, double* __restrict__ q_new, double beta) {
+__global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
+                                                   const unsigned char* __restrict__ lmask, const DevScal* __restrict__ sc,
+                                                   const double* __restrict__ dFbuf, const double* __restrict__ dFb,
+                                                   double* __restrict__ R, double* __restrict__ q_new, double beta) {
   const unsigned int n = sc->list_count;
   const double dtb = sc->dt * beta;
   for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
@@ -232,30 +315,30 @@ __global__ void __launch_bounds__(128) k_weno_apply(const __grid_constant__ DevP
     const bool skip_x = i == P.nx - 1 && P.bc[1] == BC_OUTFLOW;   // S8 replaces the x-difference there
     if (!skip_x) {
       const double ih = P.ih[0][i];
-      if (mask & 1) { weno_delta<0>(P, w, i - 1, j, k, dF);
+      if (mask & 1) { dF_below<0>(P, dFbuf, dFb, i, j, k, dF);
 #pragma unroll
         for (int v = 0; v < 5; ++v) dR[v] += ih * dF[v]; }
-      if (mask & 2) { weno_delta<0>(P, w, i, j, k, dF);
+      if (mask & 2) {
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dR[v] -= ih * dF[v]; }
+        for (int v = 0; v < 5; ++v) dR[v] -= ih * dFbuf[o + v * P.N]; }
     }
     {
       const double ih = P.ih[1][j];
-      if (mask & 4) { weno_delta<1>(P, w, i, j - 1, k, dF);
+      if (mask & 4) { dF_below<1>(P, dFbuf, dFb, i, j, k, dF);
 #pragma unroll
         for (int v = 0; v < 5; ++v) dR[v] += ih * dF[v]; }
-      if (mask & 8) { weno_delta<1>(P, w, i, j, k, dF);
+      if (mask & 8) {
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dR[v] -= ih * dF[v]; }
+        for (int v = 0; v < 5; ++v) dR[v] -= ih * dFbuf[(size_t)5 * P.N + o + v * P.N]; }
     }
     {
       const double ih = P.ih[2][k];
-      if (mask & 16) { weno_delta<2>(P, w, i, j, k - 1, dF);
+      if (mask & 16) { dF_below<2>(P, dFbuf, dFb, i, j, k, dF);
 #pragma unroll
         for (int v = 0; v < 5; ++v) dR[v] += ih * dF[v]; }
-      if (mask & 32) { weno_delta<2>(P, w, i, j, k, dF);
+      if (mask & 32) {
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dR[v] -= ih * dF[v]; }
+        for (int v = 0; v < 5; ++v) dR[v] -= ih * dFbuf[(size_t)10 * P.N + o + v * P.N]; }
     }
 #pragma unroll
     for (int v = 0; v < 5; ++v) R[o + v * P.N] += dR[v];

@@ -35,6 +35,9 @@ struct streams_ctx {
   double *qbuf[2], *S[2], *theta, *partial, *inflow, *speeds;   // qbuf: primitives [NQ][N]; S: R registers [5][N]
   unsigned char *nflag, *lmask;
   unsigned int* list;
+  unsigned int* ilist;                 // [3][N] interface lists (lower node of each flagged interface)
+  double* dFbuf;                       // [3][5][N] dF of the interface above each node (flagged entries only)
+  double* dFb;                         // dF of the interfaces below the first node of a non-periodic direction
   int npartial;
   // context-owned small device memory
   void* small_dev;
@@ -45,6 +48,7 @@ struct streams_ctx {
   long long launches;
   dim3 rhs_grid;
   int lz;
+  size_t istride;                      // entries per direction of ilist
   int dt_ready;                        // sc->dt_next holds the CFL step of the current state (last k_force_fix of a step)
   CUtensorMap tmap[2];           // TMA descriptors of qbuf[0], qbuf[1] as 4-D tensors (x, y, z, field)
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
@@ -176,7 +180,7 @@ bool make_tile_map(CUtensorMap* tm, double* q, int nx, int ny, int nz) {
 
 struct Carve { size_t off = 0; size_t take(size_t bytes) { size_t o = off; off += up(bytes); return o; } };
 
-struct Layout { size_t w[2], S[2], theta, nflag, lmask, list, partial, inflow, speeds, total; int npartial; dim3 grid; int lz; };
+struct Layout { size_t w[2], S[2], theta, nflag, lmask, list, ilist, dFbuf, dFb, partial, inflow, speeds, total; int npartial; dim3 grid; int lz; size_t istride; };
 
 Layout make_layout(const streams_grid& g, const streams_params& p) {
   Layout L;
@@ -184,12 +188,16 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   Carve c;
   for (int i = 0; i < 2; ++i) L.w[i] = c.take(NQ * N * sizeof(double));
   for (int i = 0; i < 2; ++i) L.S[i] = c.take(5 * N * sizeof(double));
-  L.theta = L.nflag = L.lmask = L.list = 0;
+  L.theta = L.nflag = L.lmask = L.list = L.ilist = L.dFbuf = L.dFb = 0;
   if (p.weno_enable) {
     L.theta = c.take(N * sizeof(double));
     L.nflag = c.take(N);
     L.lmask = c.take(N);
     L.list = c.take(N * sizeof(unsigned int));
+    L.istride = N + std::max({(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny});
+    L.ilist = c.take(3 * L.istride * sizeof(unsigned int));
+    L.dFbuf = c.take(15 * N * sizeof(double));
+    L.dFb = c.take(5 * ((size_t)g.ny * g.nz + (size_t)g.nx * g.nz + (size_t)g.nx * g.ny) * sizeof(double));
   }
   const int tiles_x = (g.nx + TX - 1) / TX, tiles_y = (g.ny + TY - 1) / TY;
   const int tiles = tiles_x * tiles_y;
@@ -306,9 +314,10 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   if (p->weno_enable) {
     c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
     c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
+    c->ilist = (unsigned int*)(base + L.ilist); c->dFbuf = (double*)(base + L.dFbuf); c->dFb = (double*)(base + L.dFb);
   }
   c->partial = (double*)(base + L.partial); c->inflow = (double*)(base + L.inflow); c->speeds = (double*)(base + L.speeds);
-  c->npartial = L.npartial; c->rhs_grid = L.grid; c->lz = L.lz;
+  c->npartial = L.npartial; c->rhs_grid = L.grid; c->lz = L.lz; c->istride = L.istride;
 
   // ---- S1 ghost coordinates and S2 metrics (host, O(n)) ----
   const int n[3] = {g->nx, g->ny, g->nz};
@@ -475,7 +484,7 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
   const int rg = rgrid_for(c->P.N);
   k_sensor<<<rg, RT, 0, c->st>>>(c->P, w, c->nflag, theta_out, c->sc);
   LAUNCH_CHECK("k_sensor");
-  k_weno_list<<<rg, RT, 0, c->st>>>(c->P, c->nflag, build_list ? c->list : nullptr, c->lmask, iflags_out, c->sc);
+  k_weno_list<<<rg, RT, 0, c->st>>>(c->P, c->nflag, build_list ? c->list : nullptr, c->lmask, nullptr, 0, iflags_out, c->sc);
   LAUNCH_CHECK("k_weno_list");
   return STREAMS_OK;
 }
@@ -483,8 +492,25 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
 // list of nodes with flagged interfaces from the node flags k_rhs has just written (a3)
 static int run_list(streams_ctx* c) {
   CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
-  k_weno_list<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->list, c->lmask, nullptr, c->sc);
+  CK(cudaMemsetAsync(&c->sc->icount[0], 0, 4 * sizeof(unsigned int), c->st));
+  k_weno_list<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->list, c->lmask, c->ilist, c->istride, nullptr, c->sc);
   LAUNCH_CHECK("k_weno_list");
+  return STREAMS_OK;
+}
+
+// a5: lists from the flags of the last k_rhs, dF once per flagged interface, then the listed nodes take
+// R += dR and (q_new != NULL) the advanced state takes dt beta dR
+static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, double beta) {
+  int rc;
+  if ((rc = run_list(c))) return rc;
+  k_weno_flux<0><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+  LAUNCH_CHECK("k_weno_flux<0>");
+  k_weno_flux<1><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+  LAUNCH_CHECK("k_weno_flux<1>");
+  k_weno_flux<2><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+  LAUNCH_CHECK("k_weno_flux<2>");
+  k_weno_apply<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->dFbuf, c->dFb, R, q_new, beta);
+  LAUNCH_CHECK("k_weno_apply");
   return STREAMS_OK;
 }
 
@@ -527,9 +553,7 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   A.partial = partial_ok ? c->partial : nullptr;
   if ((rc = launch_rhs(c, false, A))) return rc;
   if (c->p.weno_enable) {
-    if ((rc = run_list(c))) return rc;
-    k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, d_rhs, nullptr, 0.0);
-    LAUNCH_CHECK("k_weno_apply");
+    if ((rc = run_weno(c, w, d_rhs, nullptr, 0.0))) return rc;
   }
   if (c->p.forcing) {
     if ((rc = force_from_partials(c, d_rhs, partial_ok))) return rc;
@@ -595,9 +619,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
         if ((rc = launch_rhs(c, false, A))) return rc;
         if (c->p.weno_enable) {
-          if ((rc = run_list(c))) return rc;
-          k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, Sc, nullptr, 0.0);
-          LAUNCH_CHECK("k_weno_apply");
+          if ((rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
         }
         if ((rc = force_from_partials(c, Sc, partial_ok))) return rc;
         k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1, l < 2 ? 1 : 0);
@@ -609,9 +631,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
         if ((rc = launch_rhs(c, true, A))) return rc;
         if (c->p.weno_enable) {
-          if ((rc = run_list(c))) return rc;
-          k_weno_apply<<<148 * 4, 128, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->S[0], wn, beta[l]);
-          LAUNCH_CHECK("k_weno_apply");
+          if ((rc = run_weno(c, w, c->S[0], wn, beta[l]))) return rc;
         }
         c->cur ^= 1;
       }
