@@ -72,8 +72,6 @@ struct RhsArgs {
                           // previous R WITHOUT its forcing terms; they are added here as f_prev (e_rhou + u_prev e_rhoE),
                           // u_prev = the velocity still sitting in q_out (the previous stage's input state)
   double alpha, beta;
-  int lazy;               // FUSED: 1 = lazy forcing: k_force_fix rewrites u, T, mu, H of every node afterwards, so mu(T) is
-                          // not evaluated here (the power law is the longest dependency chain of the epilogue)
   int write_S;            // FUSED: 0 in the last stage (alpha of the next stage is 0: R is never read)
   unsigned char* nflag;   // hybrid switch on: node flags theta > theta_th of Eq. 8 (a3), a by-product of the velocity
                           // gradients; [N] bytes, NULL when the WENO switch is off
@@ -96,8 +94,9 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar) {
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
   unsigned ok;
   do {
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    // potentially blocking: the warp sleeps in hardware up to the time hint (ns) instead of spinning on issue slots
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity), "r"(4000u) : "memory");
   } while (!ok);
 }
 // one 4-D box (x, y, z, field) of the primitive state into a tile buffer; completes `TILE_BYTES` on the mbarrier
@@ -331,8 +330,10 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
 // special node (no staggered-wall row, no Dirichlet wall row, no characteristic outflow column), with TMA and the
 // viscous terms on: every such test folds at compile time and no out-of-line call remains in the plane loop, which
 // frees ~30 registers for the scheduler.  Ghost slots (periodic wrap, reflection, ...) are handled in both.
-template <bool FUSED, bool PLAIN>
+// MODE: 0 = residual only (streams_rhs), 1 = fused RK stage, 2 = fused RK stage with lazy forcing (mu(T) left to k_force_fix)
+template <int MODE, bool PLAIN>
 __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const CUtensorMap& tmap, double* sm) {
+  constexpr bool FUSED = MODE != 0, LAZY = MODE == 2;
   double* tiles = sm;
   double* stg = tiles + SM_TILES;
   double* gring = stg + 2 * SM_STG1;
@@ -598,9 +599,11 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
       tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
     }
-    // ================= plane p = s-3: add the z-mixed terms, write the result ====================
+    // ================= after the barrier: plane p = s-3 is completed and written (z-mixed terms, epilogue), plane s
+    // is assembled (xy mixed terms, viscous stresses) into the residual ring.  The two are independent dependency
+    // chains; on plain tiles in the interior of a chunk they sit in ONE straight block so that they interleave.
     const int p = s - 3;
-    if (active && p >= k0) {
+    auto finish_p = [&]() {
       double R[5];
       {
         const double* rr = rring + b3 * 5 * NPT + tl;               // plane s-3 sits in slot it % 3
@@ -644,24 +647,16 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
           if (A.write_S) A.S_out[o + v * P.N] = R[v];
         }
         Prim qn; qn.rho = rw[0]; qn.u = uw[0]; qn.v = vw[0]; qn.w = ww[0]; qn.T = Tw[0]; qn.mu = mw[0]; qn.H = 0.0;
-        bool store_mu = !A.lazy;
-        if (A.lazy) advance_prim<false>(P, qn, dW); else advance_prim<true>(P, qn, dW);
+        bool store_mu = !LAZY;
+        advance_prim<!LAZY>(P, qn, dW);
         if (!PLAIN && gj == 0 && P.bc[2] == BC_WALL_NODE) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
         if (!PLAIN && gj == P.ny - 1 && P.bc[3] == BC_WALL_NODE) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
         A.q_out[o] = qn.rho; A.q_out[o + P.N] = qn.u; A.q_out[o + 2 * P.N] = qn.v; A.q_out[o + 3 * P.N] = qn.w;
         A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 6 * P.N] = qn.H;
         if (store_mu) A.q_out[o + 5 * P.N] = qn.mu;
       }
-    }
-    if (active && full) {
-      if (A.nflag) {
-        // S4 / Eq. 8 (PAPER.md:81): same expression, same order as k_sensor (the flags must agree bit for bit)
-        const double* G = N.G;
-        const double div = G[0] + G[4] + G[8];
-        const double ox = G[7] - G[5], oy = G[2] - G[6], oz = G[3] - G[1];
-        const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
-        A.nflag[(size_t)s * P.nxy + own_off] = th > P.th_thr ? 1 : 0;
-      }
+        };
+    auto assemble_s = [&]() {
       if (PLAIN || P.viscous) {
         // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
         const int sy = lj * PITCH + li + XH, sx = (lj + HALO) * TX + li;
@@ -681,6 +676,24 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       double* rr = rring + b3 * 5 * NPT + tl;
 #pragma unroll
       for (int v = 0; v < 5; ++v) rr[v * NPT] = N.R[v];
+        };
+    const bool do_fin = active && p >= k0, do_asm = active && full;
+    if (PLAIN && do_fin && do_asm) {
+      finish_p();
+      assemble_s();
+    } else {
+      if (do_fin) finish_p();
+      if (do_asm) assemble_s();
+    }
+    if (do_asm) {
+      if (A.nflag) {
+        // S4 / Eq. 8 (PAPER.md:81): same expression, same order as k_sensor (the flags must agree bit for bit)
+        const double* G = N.G;
+        const double div = G[0] + G[4] + G[8];
+        const double ox = G[7] - G[5], oy = G[2] - G[6], oz = G[3] - G[1];
+        const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
+        A.nflag[(size_t)s * P.nxy + own_off] = th > P.th_thr ? 1 : 0;
+      }
     }
     slot7 = slot7 == 6 ? 0 : slot7 + 1;
     b3 = b3 == 2 ? 0 : b3 + 1;
@@ -701,7 +714,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   }
 }
 
-template <bool FUSED>
+template <int MODE>
 __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) double sm[];
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
@@ -709,8 +722,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
   const bool wall_lo = (P.bc[2] == BC_WALL_STAG || P.bc[2] == BC_WALL_NODE) && j0 == 0;
   const bool wall_hi = (P.bc[3] == BC_WALL_STAG || P.bc[3] == BC_WALL_NODE) && j0 + TY >= P.ny;
-  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<FUSED, true>(P, A, tmap, sm);
-  else rhs_body<FUSED, false>(P, A, tmap, sm);
+  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, tmap, sm);
+  else rhs_body<MODE, false>(P, A, tmap, sm);
 }
 
 }  // namespace streams

@@ -424,8 +424,9 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
         cudaFree(c->small_dev); delete c;
         return fail(nullptr, STREAMS_ECUDA, "cuTensorMapEncodeTiled failed");
       }
-  e = cudaFuncSetAttribute(k_rhs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
+  e = cudaFuncSetAttribute(k_rhs<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaFuncSetAttribute(k_rhs)"); }
   *out = c;
   return STREAMS_OK;
@@ -514,7 +515,7 @@ static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, d
   return STREAMS_OK;
 }
 
-static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A_in) {
+static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in) {
   RhsArgs A = A_in;
   A.use_tma = c->use_tma;
   A.nflag = c->p.weno_enable ? c->nflag : nullptr;
@@ -522,8 +523,9 @@ static int launch_rhs(streams_ctx* c, bool fused, const RhsArgs& A_in) {
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
-  if (fused) k_rhs<true><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);
-  else k_rhs<false><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);
+  if (mode == 2) k_rhs<2><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);       // fused RK stage, lazy forcing
+  else if (mode == 1) k_rhs<1><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);  // fused RK stage
+  else k_rhs<0><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);                 // residual only
   LAUNCH_CHECK("k_rhs");
   if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
@@ -551,7 +553,7 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   A.q = w; A.out_rhs = d_rhs; A.lz = c->lz;
   const bool partial_ok = c->p.forcing && !c->p.weno_enable;
   A.partial = partial_ok ? c->partial : nullptr;
-  if ((rc = launch_rhs(c, false, A))) return rc;
+  if ((rc = launch_rhs(c, 0, A))) return rc;
   if (c->p.weno_enable) {
     if ((rc = run_weno(c, w, d_rhs, nullptr, 0.0))) return rc;
   }
@@ -599,8 +601,8 @@ int streams_step(streams_ctx* c, int nsteps) {
         double* wn = c->qbuf[c->cur ^ 1];
         A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
         A.f_prev = l > 0 ? &c->sc->force : nullptr;
-        A.lazy = 1; A.write_S = l < 2 ? 1 : 0;
-        if ((rc = launch_rhs(c, true, A))) return rc;
+        A.write_S = l < 2 ? 1 : 0;
+        if ((rc = launch_rhs(c, 2, A))) return rc;
         if ((rc = force_from_partials(c, nullptr, true))) return rc;
         const bool want_dt = l == 2 && !(c->p.dt_fixed > 0.0);
         k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l], want_dt ? c->partial : nullptr);
@@ -617,7 +619,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         double* Sc = c->S[c->scur ^ 1];
         const bool partial_ok = !c->p.weno_enable;
         A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
-        if ((rc = launch_rhs(c, false, A))) return rc;
+        if ((rc = launch_rhs(c, 0, A))) return rc;
         if (c->p.weno_enable) {
           if ((rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
         }
@@ -629,7 +631,7 @@ int streams_step(streams_ctx* c, int nsteps) {
         // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
         double* wn = c->qbuf[c->cur ^ 1];
         A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
-        if ((rc = launch_rhs(c, true, A))) return rc;
+        if ((rc = launch_rhs(c, 1, A))) return rc;
         if (c->p.weno_enable) {
           if ((rc = run_weno(c, w, c->S[0], wn, beta[l]))) return rc;
         }
