@@ -1,19 +1,26 @@
-// k_rhs.cuh -- the fused right-hand-side kernel (rows a1,a4,a6,a7,a8,a9 of the scope table), v4.
+// k_rhs.cuh -- the fused right-hand-side kernel (rows a1,a3 (flags),a4,a6,a7,a8,a9 of the scope table).
 //
 // One CTA owns a TX x TY tile of (x,y) nodes and marches over a chunk of z planes (2.5-D
-// blocking), one thread per node, 255 registers, one CTA per SM:
+// blocking), one thread per node, ~250 registers, one CTA per SM:
 //   * the tile of plane s (seven stored primitives, halo 3, x padded to 4) is brought in by ONE
-//     TMA box copy per plane (cp.async.bulk.tensor, 4-D box x,y,z,field) two planes ahead, into a
-//     ring of three buffers, completion on an mbarrier -- no thread issues a load for the tile;
-//     TMA zero-fills outside the grid, and only tiles that touch a domain face patch their ghost
-//     slots (periodic wrap, wall reflection, inflow, shock generator) by index (S1);
-//   * x and y directions read the tile; the z direction reads REGISTER windows (planes s-3..s+3
-//     of the thread's own node), so z costs one global load per field per node;
+//     TMA box copy per plane (cp.async.bulk.tensor, 4-D box x,y,z,field) into one of two buffers,
+//     completion on an mbarrier -- no thread issues a load for the tile; plane s+2 is requested
+//     into the buffer of plane s once every thread is past its in-plane reads.  TMA zero-fills
+//     outside the grid, and only tiles that touch a domain face patch their ghost slots (periodic
+//     wrap, wall reflection, inflow, shock generator) by index (S1), one plane ahead, from a list
+//     built once per CTA;
+//   * x and y directions read the tile; the z direction reads REGISTER windows (planes s-3..s+2
+//     of the thread's own node) and the own-node ring in shared memory (planes s+3..s+5, filled
+//     by thread-private cp.async): z costs no tile and no exposed global load;
 //   * the xy mixed derivatives go through two small staging arrays (D_x u on the y-extended,
-//     D_y v on the x-extended tile); ONE __syncthreads per plane;
+//     D_y v on the x-extended tile); the ONE CTA-wide barrier per plane is split: arrive after the
+//     staging rows are written, wait after the z direction;
 //   * the z-mixed terms d_z(d_x w), d_z(d_y w), d_z(d_x u + d_y v) of plane s-3 need planes up
 //     to s, so plane s-3 is completed and written at step s ("delayed output"); the pending
-//     residuals and in-plane derivatives sit in thread-private shared-memory columns.
+//     residuals and in-plane derivatives sit in thread-private shared-memory columns;
+//   * the epilogue writes R (MODE 0) or applies Eq. 11 and writes the primitives of the new
+//     state (MODE 1; MODE 2 = lazy forcing, see RhsArgs::f_prev), R_prev prefetched by cp.async;
+//   * with the hybrid switch on, the node flags of Eq. 8 are a by-product of the velocity gradients.
 // Convective terms: Eq. 6-7 in the telescoped pair form
 //   F_{i+1/2} - F_{i-1/2} = 2 sum_l a_l [ (rho,u,phi)~_{i,l} - (rho,u,phi)~_{i-l,l} ],
 // factored per node as phi_i * sum_l (A_l - B_l) + sum_l (A_l phi_{i+l} - B_l phi_{i-l}) with
