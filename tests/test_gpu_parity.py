@@ -115,6 +115,14 @@ def P(**kw):
     return W.default_params(Rgas=1 / GAM, mu_ref=5e-3, **kw)
 
 
+def mod(wl, **kw):
+    """The same workload with some parameters replaced."""
+    import dataclasses
+    return dataclasses.replace(wl, params=dict(wl.params, **kw))
+
+
+NODE_WALLS = [W.BC_PERIODIC, W.BC_PERIODIC, W.BC_WALL_NODE, W.BC_WALL_NODE, W.BC_PERIODIC, W.BC_PERIODIC]
+
 SMALL = {
     "inviscid_ragged": lambda: W.random_periodic(40, 20, 12, params=P(viscous_enable=0)),
     "viscous_ragged": lambda: W.random_periodic(40, 20, 12, params=P()),
@@ -133,7 +141,15 @@ SMALL = {
     "channel_ragged": lambda: W.config3_channel(37, 19, 11),
     "sbli_small": lambda: W.config4_sbli(64, 40, 8, Lx=12.0),
     "sbli_ragged": lambda: W.config4_sbli(45, 30, 7, Lx=10.0),
+    # every interface WENO with non-periodic x and y: the interface lists hold N + a boundary plane of entries
+    "sbli_weno_everywhere": lambda: mod(W.config4_sbli(45, 30, 7, Lx=10.0), sensor_threshold=-1.0),
+    # forcing and the hybrid switch together (unfused fallback: k_rhs<0>, WENO correction, k_update)
+    "channel_weno_forcing": lambda: mod(W.config3_channel(37, 19, 11), weno_enable=1, sensor_threshold=0.2, sensor_eps=0.1),
+    # forcing with Dirichlet wall nodes (lazy forcing must leave the overridden wall rows alone)
+    "channel_node_walls": lambda: mod(W.config3_channel(48, 24, 16), bc=NODE_WALLS),
 }
+
+STEPPED = ["channel_ragged", "channel_weno_forcing", "channel_node_walls", "sbli_weno_everywhere", "weno_mixed", "several_tiles_and_chunks"]
 
 
 @pytest.mark.parametrize("name", list(SMALL))
@@ -144,6 +160,13 @@ def test_rhs_small(env, name):
         nflag = check_flags(env, o, g)
         if name.startswith(("weno", "sbli")):
             assert nflag > 0
+
+
+@pytest.mark.parametrize("name", STEPPED)
+def test_steps_small(env, name):
+    """Three RK3 steps of the small cases that take a different path through streams_step (lazy forcing, forcing with
+    WENO, Dirichlet wall rows, full interface lists, several chunks): state, dt, time, mass against the oracle."""
+    check_steps(env, SMALL[name](), 3)
 
 
 def test_uniform_flow_is_bitwise_steady(env):
