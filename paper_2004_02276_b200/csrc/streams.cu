@@ -96,6 +96,7 @@ const char* validate(const streams_grid* g, const streams_params* p) {
   if ((long long)g->nx * g->ny > 0x3fffffffLL) return "more than 2^30 nodes per z-plane";
   if (!(p->gamma > 1.0) || !(p->Rgas > 0.0) || !(p->Pr > 0.0)) return "gamma > 1, Rgas > 0, Pr > 0 required";
   if (p->order != 2 && p->order != 4 && p->order != 6) return "order must be 2, 4 or 6";
+  if (p->weno_enable && (long long)g->nx * g->ny * g->nz > 0x7fffffffLL) return "more than 2^31 nodes with the hybrid switch on (interface lists)";
   if (p->weno_enable && !(p->sensor_eps > 0.0)) return "sensor_eps must be > 0 (Eq. 8 is 0/0 in uniform flow otherwise)";
   if (p->visc_model != STREAMS_VISC_POWER && p->visc_model != STREAMS_VISC_SUTHERLAND) return "unknown visc_model";
   if (!(p->cfl > 0.0) && !(p->dt_fixed > 0.0)) return "cfl > 0 or dt_fixed > 0 required";
