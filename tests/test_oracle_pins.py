@@ -9,6 +9,8 @@ conditions and sympy-manufactured fields.
 import math
 from fractions import Fraction
 
+import os
+
 import numpy as np
 import pytest
 
@@ -191,6 +193,42 @@ def test_P6_rk3_order_conditions_rational():
     assert b2 * c2 ** 2 + b3 * c3 ** 2 == Fraction(1, 3) and b3 * a32 * c2 == Fraction(1, 6)
     # the printed alpha_1 = +17/60 is not even first-order consistent
     assert sum(be) + Fraction(17, 60) + al[2] != 1
+
+
+def _golden(name):
+    rows = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", name)) as f:
+        for ln in f:
+            ln = ln.split("#")[0].split()
+            if ln:
+                rows[ln[0]] = ln[1:]
+    return rows
+
+
+def test_golden_rk3_coefficients_as_printed(ob):
+    """tests/golden/rk3_coefficients.txt holds Eq. 11's coefficients as PAPER.md:99 prints them.  The printed set is
+    not consistent (sum 47/30); the adopted set differs from it in the sign of alpha_1 only, and the oracle's step on
+    dw/dt = R with R constant in time (uniform state, body force only) advances by exactly sum(alpha + beta) dt R."""
+    g = _golden("rk3_coefficients.txt")
+    ap = [Fraction(x) for x in g["alpha_printed"]]
+    bp = [Fraction(x) for x in g["beta_printed"]]
+    aa = [Fraction(x) for x in g["alpha_adopted"]]
+    assert sum(ap) + sum(bp) == Fraction(47, 30)
+    assert sum(aa) + sum(bp) == 1
+    assert [abs(x) for x in aa] == [abs(x) for x in ap] and aa[0] == ap[0] and aa[2] == ap[2] and aa[1] == -ap[1]
+    assert (aa, bp) == ([Fraction(0), Fraction(-17, 60), Fraction(-5, 12)], [Fraction(8, 15), Fraction(5, 12), Fraction(3, 4)])
+
+
+def test_golden_flow_cases_match_workloads():
+    """The seeded stand-in workloads carry the flow parameters the paper states."""
+    g = _golden("flow_cases.txt")
+    ch = W.config3_channel(16, 8, 8)
+    c_w = np.sqrt(GAM * ch.params["Rgas"] * ch.params["T_wall"][0])
+    assert abs(1.5 / c_w - float(g["channel_bulk_mach"][0])) < 1e-12          # u_b = 1.5, c_w = 1
+    sb = W.config4_sbli(32, 16, 4, Lx=6.0)
+    c_inf = np.sqrt(GAM * sb.params["Rgas"] * sb.params["fs"][4])
+    assert abs(sb.params["fs"][1] / c_inf - float(g["sbli_mach"][0])) < 1e-12
+    assert sb.params["shock_angle_deg"] == float(g["sbli_shock_generator_deg"][0])
 
 
 def test_P6_rk3_matches_butcher_tableau(ob):
