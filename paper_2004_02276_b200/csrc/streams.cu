@@ -202,9 +202,26 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   }
   const int tiles_x = (g.nx + TX - 1) / TX, tiles_y = (g.ny + TY - 1) / TY;
   const int tiles = tiles_x * tiles_y;
-  int nchunk = (2 * 148 + tiles - 1) / tiles;            // at least ~2 waves of CTAs on 148 SMs
-  nchunk = std::max(nchunk, (g.nz + 127) / 128);         // cap the chunk length
-  nchunk = std::min(nchunk, std::max(1, g.nz / 8));      // but keep the 6-plane warm-up amortised
+  // planes per CTA.  Grids with at least half a wave of tiles (148 SMs, one CTA each): about two waves of CTAs, chunks
+  // of at most LZ_MAX planes, the 6 ghost planes of a chunk amortised over >= 8 planes (measured on configs 3-5: CTAs
+  // at different z also spread the DRAM traffic better than one wave marching in lockstep).  Smaller grids cannot fill
+  // the SMs with tiles: there the chunk count minimises  waves x (lz + 3.5)  (ghost planes cost ~40 % of a full one).
+  int nchunk;
+  if (tiles >= 74) {
+    nchunk = (2 * 148 + tiles - 1) / tiles;
+    nchunk = std::max(nchunk, (g.nz + LZ_MAX - 1) / LZ_MAX);
+    nchunk = std::min(nchunk, std::max(1, g.nz / 8));
+  } else {
+    nchunk = 1;
+    double best = 1e300;
+    for (int c = (g.nz + LZ_MAX - 1) / LZ_MAX; c <= g.nz; ++c) {
+      const int lz = (g.nz + c - 1) / c;
+      const int cc = (g.nz + lz - 1) / lz;
+      const double cost = std::ceil((double)tiles * cc / 148.0) * (lz + 3.5);
+      if (cost < best) { best = cost; nchunk = cc; }
+      if (lz == 1) break;
+    }
+  }
   L.lz = (g.nz + nchunk - 1) / nchunk;
   nchunk = (g.nz + L.lz - 1) / L.lz;
   L.grid = dim3(tiles_x, tiles_y, nchunk);
