@@ -339,7 +339,7 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
 // frees ~30 registers for the scheduler.  Ghost slots (periodic wrap, reflection, ...) are handled in both.
 // MODE: 0 = residual only (streams_rhs), 1 = fused RK stage, 2 = fused RK stage with lazy forcing (mu(T) left to k_force_fix)
 template <int MODE, bool PLAIN>
-__device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const CUtensorMap& tmap, double* sm) {
+__device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const CUtensorMap& tmap, double* sm, const int3 cta) {
   constexpr bool FUSED = MODE != 0, LAZY = MODE == 2;
   double* tiles = sm;
   double* stg = tiles + SM_TILES;
@@ -363,9 +363,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 
   const int tid = threadIdx.x;
   const int ti = tid & (TX - 1), tj = tid / TX;
-  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const int i0 = cta.x * TX, j0 = cta.y * TY;
   const int gi = i0 + ti, gj = j0 + tj;
-  const int k0 = blockIdx.z * A.lz;
+  const int k0 = cta.z * A.lz;
   const int k1 = min(k0 + A.lz, P.nz);
   const bool active = PLAIN || (gi < P.nx && gj < P.ny);
   const int oc = (tj + HALO) * PITCH + ti + XH;                               // own tile offset
@@ -717,20 +717,25 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   if (A.partial) {
     const double hxy = active ? P.hh[0][gi] * P.hh[1][gj] : 0.0;
     const double tot = block_sum<NT>(fsum * hxy, red, tid);
-    if (tid == 0) A.partial[(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = tot;
+    if (tid == 0) A.partial[(cta.z * gridDim.y + cta.y) * gridDim.x + cta.x] = tot;
   }
 }
 
 template <int MODE>
 __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) double sm[];
-  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  // CTA -> (tile, chunk): the chunk index varies fastest with the launch order, so that the CTAs resident at any time
+  // march through different z ranges (spreads the DRAM traffic; one wave in lockstep through z measured 24 % slower)
+  const int lin = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+  const int tix = lin / gridDim.z;
+  const int3 cta = make_int3(tix % gridDim.x, tix / gridDim.x, lin % gridDim.z);
+  const int i0 = cta.x * TX, j0 = cta.y * TY;
   const bool inside = i0 + TX <= P.nx && j0 + TY <= P.ny;
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
   const bool wall_lo = (P.bc[2] == BC_WALL_STAG || P.bc[2] == BC_WALL_NODE) && j0 == 0;
   const bool wall_hi = (P.bc[3] == BC_WALL_STAG || P.bc[3] == BC_WALL_NODE) && j0 + TY >= P.ny;
-  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, tmap, sm);
-  else rhs_body<MODE, false>(P, A, tmap, sm);
+  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, tmap, sm, cta);
+  else rhs_body<MODE, false>(P, A, tmap, sm, cta);
 }
 
 }  // namespace streams
