@@ -160,10 +160,11 @@ __device__ __forceinline__ double weno5(double a, double b, double c, double d, 
   const double b0 = (13.0 / 12.0) * t0 * t0 + 0.25 * u0 * u0;
   const double b1 = (13.0 / 12.0) * t1 * t1 + 0.25 * u1 * u1;
   const double b2 = (13.0 / 12.0) * t2 * t2 + 0.25 * u2 * u2;
+  // WENO-JS weights a_k = d_k / (eps + b_k)^2 (ref. [34]), written over the common denominator e0 e1 e2 so that the
+  // interface costs one division instead of four: w_k = d_k prod_{j != k} e_j, result = sum w_k q_k / sum w_k
   const double eps = 1e-6;
-  const double a0 = 0.1 / ((eps + b0) * (eps + b0));
-  const double a1 = 0.6 / ((eps + b1) * (eps + b1));
-  const double a2 = 0.3 / ((eps + b2) * (eps + b2));
+  const double e0 = (eps + b0) * (eps + b0), e1 = (eps + b1) * (eps + b1), e2 = (eps + b2) * (eps + b2);
+  const double a0 = 0.1 * (e1 * e2), a1 = 0.6 * (e0 * e2), a2 = 0.3 * (e0 * e1);
   return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
 }
 
