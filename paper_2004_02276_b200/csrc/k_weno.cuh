@@ -101,8 +101,15 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
     if (in) {
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        const int lo = iface_flag(P, nflag, d, i, j, k, id[d] - 1);
-        const int hi = iface_flag(P, nflag, d, i, j, k, id[d]);
+        // interfaces id-1/2 and id+1/2 look at nodes id-3..id+2 and id-2..id+3: one pass over the seven node flags
+        const int n = d == 0 ? P.nx : (d == 1 ? P.ny : P.nz);
+        int fl[7];
+#pragma unroll
+        for (int g = 0; g < 7; ++g) fl[g] = nflag_at(P, nflag, d, i, j, k, id[d] - 3 + g);
+        int lo = fl[0] | fl[1] | fl[2] | fl[3] | fl[4] | fl[5];
+        int hi = fl[1] | fl[2] | fl[3] | fl[4] | fl[5] | fl[6];
+        if (id[d] == 0 && P.bc[2 * d] == BC_WALL_STAG) lo = 0;            // the staggered wall plane is never flagged (A6)
+        if (id[d] == n - 1 && P.bc[2 * d + 1] == BC_WALL_STAG) hi = 0;
         mask |= (lo << (2 * d)) | (hi << (2 * d + 1));
         cnt[d] += hi;
         if (id[d] == 0 && P.bc[2 * d] != BC_PERIODIC) cnt[d] += lo;
