@@ -153,7 +153,7 @@ __device__ __forceinline__ int map_z(const DevP& P, int k) {
 // (= jj*nx+ii inside a plane), 2 the frozen inflow plane (off = jj), 3 / 4 the free-stream / post-shock
 // constant of the shock generator; kind >> 4: 0 plain, 1 / 2 isothermal reflection about wall 0 / 1.
 struct Src { int off, kind; };
-enum { SRC_NONE = 0, SRC_FIELD = 1, SRC_INFLOW = 2, SRC_FS = 3, SRC_POST = 4 };
+enum { SRC_NONE = 0, SRC_FIELD = 1, SRC_INFLOW = 2, SRC_FS = 3, SRC_POST = 4, SRC_LOCAL = 8 /* k_rhs patch list: source inside the tile */ };
 
 __device__ __forceinline__ Src resolve_xy(const DevP& P, int i, int j) {
   Src s;

@@ -224,7 +224,14 @@ __device__ __noinline__ void build_patch_list(const DevP& P, int i0, int j0, boo
     const int gi = i0 + io, gj = j0 + jo;
     if (gi >= P.nx + HALO || gj >= P.ny + HALO) continue;
     if (!all && gi >= 0 && gi < P.nx && gj >= 0 && gj < P.ny) continue;      // TMA brings it
-    const Src s = resolve_xy(P, gi, gj);
+    Src s = resolve_xy(P, gi, gj);
+    if (!all && (s.kind & 7) == SRC_FIELD) {
+      // a source node that lies inside this tile's own box (the mirror rows of a wall) is read from the tile in shared
+      // memory, not from global memory: kind bit 3, off = tile slot of the source
+      const int jj = s.off / P.nx, ii = s.off - jj * P.nx;
+      const int lo = ii - i0, ljs = jj - j0;
+      if (lo >= -XH && lo < TX + XH && ljs >= -HALO && ljs < TY + HALO) { s.kind |= SRC_LOCAL; s.off = (ljs + HALO) * PITCH + lo + XH; }
+    }
     const int n = atomicAdd(count, 1);
     list[n] = make_int2(e | (s.kind << 16), s.off);
   }
@@ -236,7 +243,13 @@ __device__ __noinline__ void patch_tile(const DevP& P, const double* __restrict_
     const int2 en = list[e];
     Src s; s.kind = en.x >> 16; s.off = en.y;
     Prim q;
-    load_src_raw(P, Q, s, kk, q);
+    if (s.kind & SRC_LOCAL) {
+      const double* r = t + s.off;
+      q.rho = r[F_RHO * TILE]; q.u = r[F_U * TILE]; q.v = r[F_V * TILE]; q.w = r[F_W * TILE];
+      q.T = r[F_T * TILE]; q.mu = r[F_MU * TILE]; q.H = r[F_H * TILE];
+    } else {
+      load_src_raw(P, Q, s, kk, q);
+    }
     apply_reflect(P, s, q);
     double* d = t + (en.x & 0xffff);
     d[F_RHO * TILE] = q.rho; d[F_U * TILE] = q.u; d[F_V * TILE] = q.v; d[F_W * TILE] = q.w;
