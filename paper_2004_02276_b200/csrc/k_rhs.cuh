@@ -386,7 +386,6 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   const int k0 = cta.z * A.lz;
   const int k1 = min(k0 + A.lz, P.nz);
   const bool active = PLAIN || (gi < P.nx && gj < P.ny);
-  const int oc = (tj + HALO) * PITCH + ti + XH;                               // own tile offset
   const int own_off = gj * P.nx + gi;
   const bool use_tma = PLAIN || A.use_tma != 0;
   // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
