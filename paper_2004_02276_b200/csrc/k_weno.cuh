@@ -95,7 +95,9 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
   for (long long it = 0; it < nround; ++it) {
     const long long o = (it * gridDim.x + blockIdx.x) * (long long)RT + threadIdx.x;
     const bool in = o < P.N;
-    const int i = in ? (int)(o % P.nx) : 0, j = in ? (int)((o / P.nx) % P.ny) : 0, k = in ? (int)(o / P.nxy) : 0;
+    // 32-bit index arithmetic: N < 2^31 with the hybrid switch on (validate())
+    const unsigned int o32 = in ? (unsigned int)o : 0u, row = o32 / (unsigned int)P.nx;
+    const int i = (int)(o32 - row * (unsigned int)P.nx), k = (int)(row / (unsigned int)P.ny), j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
     const int id[3] = {i, j, k};
     int mask = 0;
     if (in) {
@@ -274,8 +276,8 @@ __global__ void __launch_bounds__(128) k_weno_flux(const __grid_constant__ DevP 
   for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
     const unsigned int en = li[e];
     const bool below = (en & IFACE_BELOW) != 0;
-    const long long o = en & ~IFACE_BELOW;
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    const unsigned int o = en & ~IFACE_BELOW, row = o / (unsigned int)P.nx;
+    const int i = (int)(o - row * (unsigned int)P.nx), k = (int)(row / (unsigned int)P.ny), j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
     double dF[5];
     weno_delta<D>(P, w, i - (below && D == 0), j - (below && D == 1), k - (below && D == 2), dF);
     if (below) {
@@ -315,9 +317,9 @@ __global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP 
   const unsigned int n = sc->list_count;
   const double dtb = sc->dt * beta;
   for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
-    const long long o = list[e];
+    const unsigned int o = list[e], row = o / (unsigned int)P.nx;
     const int mask = lmask[e];
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    const int i = (int)(o - row * (unsigned int)P.nx), k = (int)(row / (unsigned int)P.ny), j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
     double dR[5] = {0, 0, 0, 0, 0};
     double dF[5];
     const bool skip_x = i == P.nx - 1 && P.bc[1] == BC_OUTFLOW;   // S8 replaces the x-difference there
