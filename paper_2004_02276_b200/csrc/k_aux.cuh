@@ -6,6 +6,14 @@ namespace streams {
 
 constexpr int RT = 256;                 // threads of the light grid-stride kernels
 
+// node index -> (i, j, k) in 32-bit arithmetic (validate(): N < 2^32)
+__device__ __forceinline__ void node_ijk(const DevP& P, long long o, int& i, int& j, int& k) {
+  const unsigned int o32 = (unsigned int)o, row = o32 / (unsigned int)P.nx;
+  i = (int)(o32 - row * (unsigned int)P.nx);
+  k = (int)(row / (unsigned int)P.ny);
+  j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
+}
+
 // device scalars kept between kernels (no host round trip inside streams_step)
 struct DevScal {
   double dt;            // S10
@@ -65,7 +73,8 @@ __global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, d
       dW[v] = dt * (alpha * sp + beta * r[v]);
     }
     advance_prim(P, q, dW);
-    const int j = (int)((o / P.nx) % P.ny);
+    int i_, j, k_;
+    node_ijk(P, o, i_, j, k_);
     if (j == 0 && P.bc[2] == BC_WALL_NODE) wall_node_override(P, P.Twall[0], P.mu_wall[0], q);
     if (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE) wall_node_override(P, P.Twall[1], P.mu_wall[1], q);
     Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu; Q[o + 6 * P.N] = q.H;
@@ -151,7 +160,8 @@ __global__ void __launch_bounds__(RT) k_force_partial(const __grid_constant__ De
   __shared__ double sh[RT / 32];
   double acc = 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    int i, j, k;
+    node_ijk(P, o, i, j, k);
     acc += R[o + P.N] * (P.hh[0][i] * P.hh[1][j] * P.hh[2][k]);
   }
   const double t = block_sum<RT>(acc, sh, threadIdx.x);
@@ -171,7 +181,8 @@ __global__ void __launch_bounds__(RT) k_speed_partial(const __grid_constant__ De
   __shared__ double sh[RT / 32];
   double m[3] = {0.0, 0.0, 0.0};
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    int i, j, k;
+    node_ijk(P, o, i, j, k);
     const double cs = sqrt(P.gam * P.Rgas * Q[o + 4 * P.N]);
     m[0] = fmax(m[0], (fabs(Q[o + P.N]) + cs) * P.ih[0][i]);
     m[1] = fmax(m[1], (fabs(Q[o + 2 * P.N]) + cs) * P.ih[1][j]);
@@ -205,7 +216,8 @@ __global__ void __launch_bounds__(RT) k_diag_partial(const __grid_constant__ Dev
   double s[7] = {0, 0, 0, 0, 0, 0, 0};
   double mnr = INFINITY, mnp = INFINITY, mxm = 0.0, bad = 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
-    const int i = (int)(o % P.nx), j = (int)((o / P.nx) % P.ny), k = (int)(o / P.nxy);
+    int i, j, k;
+    node_ijk(P, o, i, j, k);
     const double vol = P.hh[0][i] * P.hh[1][j] * P.hh[2][k];
     Prim q;
     q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
