@@ -238,6 +238,29 @@ def test_fp64_peak_probe_and_step_repeatability(env):
     assert all(np.isfinite(o).all() for o in outs)
 
 
+def test_split_stepping_is_bitwise_the_same(env):
+    """streams_step(5) == streams_step(2); diagnostics; streams_step(3): the CFL step carried from the last stage of a step
+    (dt_next), the lazy body force and the ping-pong buffers survive call boundaries and a diagnostics pass in between."""
+    torch, binding, ob = env
+    for wl in (SMALL["channel_small"](), SMALL["weno_mixed"](), SMALL["channel_weno_forcing"]()):
+        w0 = torch.from_numpy(wl.state()).cuda()
+        a = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+        a.set_state(w0)
+        a.step(5)
+        b = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+        b.set_state(w0)
+        b.step(2)
+        d = b.diagnostics()
+        assert d.step == 2
+        b.rhs()                                           # a residual evaluation in between must not disturb the state
+        b.step(3)
+        assert np.array_equal(a.get_state().cpu().numpy(), b.get_state().cpu().numpy()), wl.name
+        da, db = a.diagnostics(), b.diagnostics()
+        assert da.time == db.time and da.dt == db.dt and da.step == db.step == 5
+        a.close()
+        b.close()
+
+
 def test_sod_tube_gpu(env):
     """Hybrid recipe end to end on the GPU along x: same answer as the oracle after the full run."""
     n = 200
