@@ -27,7 +27,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2004_02276_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 
 METRIC = "fp64 grid-point updates/s per RK3 step"
 UNIT = "points/s"

@@ -62,6 +62,9 @@ def lib():
         L.oracle_get_metrics.argtypes = [C.c_void_p, C.c_int, _DBL, _DBL]
         L.oracle_get_sensor.argtypes = [C.c_void_p, _DBL, C.POINTER(C.c_ubyte)]
         L.oracle_get_prims.argtypes = [C.c_void_p, _DBL]
+        L.oracle_get_ghosted.argtypes = [C.c_void_p, _DBL]
+        L.oracle_roe_state.argtypes = [C.c_double, _DBL, C.c_double, C.c_double, _DBL, C.c_double, _DBL, _DBL]
+        L.oracle_roe_state.restype = None
         _lib = L
     return _lib
 
@@ -104,6 +107,15 @@ def eigen(d, gamma, ubar, Hbar):
     lam = np.zeros(5)
     lib().oracle_eigen(d, gamma, _p(ub), Hbar, _p(Lm), _p(Rm), _p(lam))
     return Lm, Rm, lam
+
+
+def roe_state(rho_a, u_a, H_a, rho_b, u_b, H_b):
+    ua = np.ascontiguousarray(u_a, dtype=np.float64)
+    ub = np.ascontiguousarray(u_b, dtype=np.float64)
+    out = np.zeros(3)
+    Hb = C.c_double(0.0)
+    lib().oracle_roe_state(rho_a, _p(ua), H_a, rho_b, _p(ub), H_b, _p(out), C.byref(Hb))
+    return out, Hb.value
 
 
 def shock_state(params: dict):
@@ -192,6 +204,12 @@ class Oracle:
         fl = np.empty((3,) + self.shape[1:], dtype=np.uint8)
         self._chk(lib().oracle_get_sensor(self._h, _p(th), fl.ctypes.data_as(C.POINTER(C.c_ubyte))))
         return th, fl
+
+    def ghosted(self):
+        """Ghost-filled conservative state [5][nz+6][ny+6][nx+6] (S1)."""
+        wg = np.empty((5, self.n[2] + 6, self.n[1] + 6, self.n[0] + 6))
+        self._chk(lib().oracle_get_ghosted(self._h, _p(wg)))
+        return wg
 
     def prims(self):
         q = np.empty((9,) + self.shape[1:])

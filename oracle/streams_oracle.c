@@ -8,16 +8,22 @@
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): coefficient tables against polynomial
- * exactness; flux form against the telescoped pair form; bitwise free-stream
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_pins_bc.py, -m "not gpu"): coefficient tables against
+ * polynomial exactness; flux form against the telescoped pair form; bitwise free-stream
  * preservation; discrete conservation; kinetic-energy identity; RK3 amplification
- * polynomial and order; eigenvectors against a complex-step Jacobian; WENO5 linear
- * limit and order; Sod tube against the exact Riemann solution; oblique-shock jump
- * conditions; metric and viscous operators against sympy-manufactured fields.
- * PARITY UNPINNED (choices of DESIGN.md only, nothing in the paper fixes them):
- * sensor threshold / regulariser values, the boundary closures A13-A17 (frozen inflow,
- * non-reflecting outflow formula, sharp shock-generator jump, nearest-node theta at
- * non-periodic ghosts), and the CFL definition S10.
+ * polynomial, Butcher tableau and order (coefficients read from tests/golden/); eigenvectors
+ * against a complex-step Jacobian; Roe state against Roe's property U and a moving-shock
+ * closed form of the WENO flux; WENO5 linear limit and order; Sod tube against the exact
+ * Riemann solution; oblique-shock jump conditions; metric and viscous operators against
+ * sympy-manufactured fields; wall ghost rules (staggered and node) against hand-built ghosts
+ * and the closed forms of linear profiles continued through the wall; Dirichlet wall-node
+ * override; shock-generator ghost rows and the residual they produce; frozen-inflow ghosts
+ * and the x -> y -> z corner fill order; Sutherland's law; the sensor of Eq. 8 on a
+ * manufactured field with all nine velocity gradients; the f u_1 power of Eq. 1c.
+ * PARITY UNPINNED (choices of DESIGN.md only, nothing in the paper fixes them): the VALUES of
+ * the sensor threshold / regulariser, the non-reflecting outflow formula A13 beyond "uniform
+ * flow gives 0, a pulse leaves" (P14), nearest-node theta at non-periodic ghosts (A17), and the
+ * CFL definition S10 beyond its closed form on a uniform state (P13).
  */
 #include "streams_oracle.h"
 
@@ -500,6 +506,15 @@ void oracle_eigen(int d, double gam, const double ub[3], double Hb, double Lm[25
   lam[0] = un - cs; lam[1] = un; lam[2] = un; lam[3] = un; lam[4] = un + cs;
 }
 
+/* S6 step 1: Roe state of two nodes a (lower) and b (upper): r = sqrt(rho_b / rho_a), square-root-of-density
+ * weighted means of the velocity components and of the total enthalpy */
+void oracle_roe_state(double rho_a, const double u_a[3], double H_a, double rho_b, const double u_b[3], double H_b,
+                      double ubar[3], double* Hbar) {
+  const double r = sqrt(rho_b / rho_a);
+  for (int m = 0; m < 3; ++m) ubar[m] = (u_a[m] + r * u_b[m]) / (1.0 + r);
+  *Hbar = (H_a + r * H_b) / (1.0 + r);
+}
+
 /* S6: characteristic-wise Lax-Friedrichs split WENO5 flux at interface i+1/2 */
 static void weno_flux(const oracle_ctx* c, int d, size_t o, double F[5]) {
   const size_t NP = c->NP, s = c->sd[d];
@@ -507,10 +522,10 @@ static void weno_flux(const oracle_ctx* c, int d, size_t o, double F[5]) {
   const double* Q = c->q;
   /* 1. Roe state from nodes i, i+1 */
   const size_t oa = o, ob = o + s;
-  const double r = sqrt(Q[Q_RHO * NP + ob] / Q[Q_RHO * NP + oa]);
-  double ub[3];
-  for (int m = 0; m < 3; ++m) ub[m] = (Q[(Q_U + m) * NP + oa] + r * Q[(Q_U + m) * NP + ob]) / (1.0 + r);
-  const double Hb = (Q[Q_H * NP + oa] + r * Q[Q_H * NP + ob]) / (1.0 + r);
+  const double ua[3] = {Q[Q_U * NP + oa], Q[Q_V * NP + oa], Q[Q_W * NP + oa]};
+  const double ubn[3] = {Q[Q_U * NP + ob], Q[Q_V * NP + ob], Q[Q_W * NP + ob]};
+  double ub[3], Hb;
+  oracle_roe_state(Q[Q_RHO * NP + oa], ua, Q[Q_H * NP + oa], Q[Q_RHO * NP + ob], ubn, Q[Q_H * NP + ob], ub, &Hb);
   /* 2. eigenvectors */
   double Lm[25], Rm[25], lamb[5];
   oracle_eigen(d, gam, ub, Hb, Lm, Rm, lamb);
@@ -754,6 +769,15 @@ int oracle_get_prims(oracle_ctx* c, double* out) {
     for (int k = 0; k < c->n[2]; ++k)
       for (int j = 0; j < c->n[1]; ++j)
         for (int i = 0; i < c->n[0]; ++i) out[v * c->np + II(c, i, j, k)] = c->q[v * c->NP + GI(c, i, j, k)];
+  return ORC_OK;
+}
+
+/* accessor for the pins of S1: the ghost-filled conservative state [5][nz+6][ny+6][nx+6] of the current state */
+int oracle_get_ghosted(oracle_ctx* c, double* wg_out) {
+  if (!c || !wg_out) return ORC_EINVAL;
+  if (!c->has_state) return ORC_ESTATE;
+  fill_ghosts(c);
+  memcpy(wg_out, c->wg, NV * c->NP * sizeof(double));
   return ORC_OK;
 }
 

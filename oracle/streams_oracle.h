@@ -66,6 +66,9 @@ int  oracle_get_metrics(oracle_ctx*, int d, double* h_out, double* g_out);  /* S
 int  oracle_get_sensor(oracle_ctx*, double* theta_out, unsigned char* flags_out); /* S4: theta[nz][ny][nx], flags[3][nz][ny][nx] */
 int  oracle_get_prims(oracle_ctx*, double* prim_out);                       /* S3: [9][nz][ny][nx] rho,u,v,w,p,T,H,c,mu */
 int  oracle_rhs_parts(oracle_ctx*, double* conv_out, double* visc_out);     /* convective / viscous split of R (no forcing) */
+int  oracle_get_ghosted(oracle_ctx*, double* wg_out);                       /* S1: ghost-filled state [5][nz+6][ny+6][nx+6] */
+void oracle_roe_state(double rho_a, const double u_a[3], double H_a, double rho_b, const double u_b[3], double H_b,
+                      double ubar[3], double* Hbar);                        /* S6 step 1               */
 
 #ifdef __cplusplus
 }

@@ -16,7 +16,7 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, S
 
 EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
-           "streams_diagnostics", "streams_profile", "streams_profile_read", "streams_launch_count", "streams_last_error", "streams_destroy"]
+           "streams_diagnostics", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
 
 
 class StreamsGrid(C.Structure):

@@ -22,7 +22,7 @@ def blib():
 
 def test_exports_every_declared_symbol(blib):
     src = open(HEADER).read()
-    declared = set(re.findall(r"\b(streams_[a-z_]+)\s*\(", src))
+    declared = set(re.findall(r"\b(streams_[a-z0-9_]+)\s*\(", src))
     assert declared, "no prototypes found"
     L = blib.lib()
     for name in sorted(declared):
@@ -54,7 +54,7 @@ int main(void){
 
 
 def test_workspace_and_validation(blib):
-    from paper_2004_02276_b200 import workloads as W
+    import workloads as W
     wl = W.config3_channel(256, 128, 128)
     n = wl.npoints
     nb = blib.workspace_bytes(wl.grid, wl.params)
@@ -86,7 +86,7 @@ def test_product_never_imports_oracle():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
-                assert "oracle" not in txt.lower() or f == "workloads.py", f
+                assert "oracle" not in txt.lower(), f
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".c", ".h")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()

@@ -11,7 +11,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2004_02276_b200 import workloads as W
+import workloads as W
 
 pytestmark = pytest.mark.gpu
 GAM = 1.4

@@ -14,7 +14,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2004_02276_b200 import workloads as W
+import workloads as W
 from tests import helpers as H
 
 GAM = 1.4
@@ -207,8 +207,9 @@ def _golden(name):
 
 def test_golden_rk3_coefficients_as_printed(ob):
     """tests/golden/rk3_coefficients.txt holds Eq. 11's coefficients as PAPER.md:99 prints them.  The printed set is
-    not consistent (sum 47/30); the adopted set differs from it in the sign of alpha_1 only, and the oracle's step on
-    dw/dt = R with R constant in time (uniform state, body force only) advances by exactly sum(alpha + beta) dt R."""
+    not consistent (sum 47/30); the adopted set differs from it in the sign of alpha_1 only.  One oracle step must be
+    Eq. 11 written out with the coefficients OF THE FILE (beta as printed, alpha with the sign reading) around the
+    oracle's own R(w): w1 = w0 + dt b0 R0, w2 = w1 + dt (a1 R0 + b1 R1), w3 = w2 + dt (a2 R1 + b2 R2)."""
     g = _golden("rk3_coefficients.txt")
     ap = [Fraction(x) for x in g["alpha_printed"]]
     bp = [Fraction(x) for x in g["beta_printed"]]
@@ -217,6 +218,30 @@ def test_golden_rk3_coefficients_as_printed(ob):
     assert sum(aa) + sum(bp) == 1
     assert [abs(x) for x in aa] == [abs(x) for x in ap] and aa[0] == ap[0] and aa[2] == ap[2] and aa[1] == -ap[1]
     assert (aa, bp) == ([Fraction(0), Fraction(-17, 60), Fraction(-5, 12)], [Fraction(8, 15), Fraction(5, 12), Fraction(3, 4)])
+    al, be = [float(x) for x in aa], [float(x) for x in bp]
+    dt = 0.01
+    wl = W.config1_tgv(8, weno=0)
+    wl.params.update(dt_fixed=dt)
+    o = make(ob, wl)
+    w = wl.state()
+    r_prev = np.zeros_like(w)
+    for l in range(3):
+        o.set_state(w)
+        r = o.rhs()
+        w = w + dt * (al[l] * r_prev + be[l] * r)
+        r_prev = r
+    o.set_state(wl.state())
+    o.step(1)
+    assert np.max(np.abs(o.get_state() - w)) < 1e-13 * np.abs(w).max()
+    # with alpha_1 as printed the same recurrence lands somewhere else (first-order inconsistent)
+    w_bad = wl.state()
+    r_prev = np.zeros_like(w_bad)
+    for l in range(3):
+        o.set_state(w_bad)
+        r = o.rhs()
+        w_bad = w_bad + dt * (float(ap[l]) * r_prev + be[l] * r)
+        r_prev = r
+    assert np.max(np.abs(w_bad - w)) > 1e-6 * np.abs(w).max()
 
 
 def test_golden_flow_cases_match_workloads():
