@@ -114,28 +114,38 @@ typedef struct {
   int pad_;
 } streams_diag;
 
-/* Bytes of device workspace `streams_create` needs for this grid/params (0 on bad input). */
+/* Bytes of device workspace `streams_create` needs for this grid/params (0 on bad input).
+ * Passage: PAPER.md:183-225 (section 4.2: the state array w_gpu and the RK increment array fln_gpu live in
+ * device memory for the whole time loop); here the caller owns that memory. */
 size_t streams_workspace_bytes(const streams_grid* grid, const streams_params* params);
 
-/* Create a context.  h_x/h_y/h_z: HOST arrays of nx/ny/nz node coordinates, strictly
+/* Create a context for one Cartesian grid, stretched or uniform per direction (PAPER.md:110 error-function /
+ * PAPER.md:124 hyperbolic-sine wall-normal mappings are the caller's: the library takes node coordinates and forms
+ * the metrics of Eq. 5 generalised to non-uniform spacing, S2), gas model (Eq. 2-3),
+ * scheme order, boundary kinds and forcing.
+ * h_x/h_y/h_z: HOST arrays of nx/ny/nz node coordinates, strictly
  * increasing.  d_workspace: DEVICE memory, >= streams_workspace_bytes(), 256-B aligned,
  * owned by the caller.  cuda_stream: cudaStream_t as void*.  On success *out is set. */
 int streams_create(const streams_grid* grid, const double* h_x, const double* h_y, const double* h_z,
                    const streams_params* params, void* d_workspace, size_t workspace_bytes,
                    void* cuda_stream, streams_ctx** out);
 
-/* Copy a state into the context (device->device, async).  Captures the frozen inflow
+/* Copy a state w = [rho, rho u, rho v, rho w, rho E] (Eq. 10) into the context: the paper's
+ * `w_gpu = w`.  Device->device, async; converts to the stored primitives.  Captures the frozen inflow
  * plane when bc[xmin] == INFLOW_FROZEN.  Resets step counter, time and RK register. */
 int streams_set_state(streams_ctx* ctx, const double* d_w);
 /* Same from pageable or pinned HOST memory (host->device copy on the context stream; synchronises). */
 int streams_set_state_host(streams_ctx* ctx, const double* h_w);
 
-/* Copy the current state out (device->device, async). */
+/* Copy the current conservative state w out: the paper's `w = w_gpu`.  Device->device, async. */
 int streams_get_state(streams_ctx* ctx, double* d_w_out);
 /* Same into HOST memory (synchronises). */
 int streams_get_state_host(streams_ctx* ctx, double* h_w_out);
 
-/* R(w) of the current state into d_rhs_out ([5][nz][ny][nx]); includes the body force
+/* The residual vector R(w) of Eq. 10: convective terms by the energy-preserving central flux of
+ * Eq. 5-7 or, on interfaces flagged by the sensor of Eq. 8, the characteristic
+ * Lax-Friedrichs WENO flux; viscous terms in the Laplacian form of Eq. 9.
+ * R of the current state goes into d_rhs_out ([5][nz][ny][nx]); includes the body force
  * (forcing=1) and the characteristic replacement at OUTFLOW_NR nodes, excludes the
  * Dirichlet node overrides of NODE walls.  State, time and step counter unchanged. */
 int streams_rhs(streams_ctx* ctx, double* d_rhs_out);
@@ -145,13 +155,31 @@ int streams_rhs(streams_ctx* ctx, double* d_rhs_out);
  * receives 1 where interface i+1/2 (resp. j+1/2, k+1/2) above node (i,j,k) is flagged. */
 int streams_sensor(streams_ctx* ctx, double* d_theta_out, unsigned char* d_flags_out);
 
-/* Advance nsteps full RK3 steps (Eq. 11); dt recomputed on the device every step
- * unless dt_fixed > 0.  No host synchronisation. */
+/* Advance nsteps full steps of Wray's three-stage scheme, Eq. 11 (alpha_1 = -17/60, G5);
+ * dt recomputed on the device every step unless dt_fixed > 0 (S10); the body force is re-evaluated at every
+ * stage.  No host synchronisation.  On a stream of the caller's own (not the legacy default
+ * stream) grids below 2^24 nodes replay one captured CUDA graph per step instead of launching kernel by kernel. */
 int streams_step(streams_ctx* ctx, int nsteps);
 
-/* Reductions of the current state into *h_out (host struct).  Synchronises.  Returns
+/* Reductions of the current state into *h_out (host struct): the volume integrals of PAPER.md:107 (bulk density
+ * rho_b = 1/V int rho dV and bulk momentum, "both exactly constant in time"), total energy and kinetic energy
+ * (PAPER.md:77), the last body force f, extrema and sensor statistics (Eq. 8).  Synchronises.  Returns
  * STREAMS_ENONFINITE (with *h_out filled) if the state is not physical. */
 int streams_diagnostics(streams_ctx* ctx, streams_diag* h_out);
+
+/* Reynolds / Favre statistics ("the overline symbol denotes averaging in the homogeneous space
+ * directions and in time"; phi~ = mean(rho phi) / mean(rho)).  streams_stats_accumulate adds the x-z plane means
+ * (plain node means: x and z are the homogeneous, uniformly spaced directions) of the current state to running sums
+ * on the device, one profile over the wall-normal index j per quantity; async, no host synchronisation.
+ * streams_stats_read returns the time average (sums / samples) into h_out[STREAMS_NSTAT][ny] (HOST) and the number
+ * of samples; synchronises.  Order of the quantities:
+ *   rho, u, v, w, p, T, mu, rho u, rho v, rho w, rho T, rho u u, rho v v, rho w w, rho u v, T T
+ * e.g. Favre mean u~ = out[7]/out[0]; density-scaled stress rho u''u'' = out[11] - out[7]^2/out[0] (Fig. 3).
+ * streams_stats_reset clears sums and sample count. */
+enum { STREAMS_NSTAT = 16 };
+int streams_stats_accumulate(streams_ctx* ctx);
+int streams_stats_read(streams_ctx* ctx, double* h_out, long long* h_nsamples);
+int streams_stats_reset(streams_ctx* ctx);
 
 /* Kernel timing for roofline accounting.  streams_profile(ctx, 1) clears the record and makes
  * every following launch of the fused RHS kernel (k_rhs) be bracketed by CUDA events on the

@@ -62,6 +62,9 @@ def lib():
         L.oracle_get_metrics.argtypes = [C.c_void_p, C.c_int, _DBL, _DBL]
         L.oracle_get_sensor.argtypes = [C.c_void_p, _DBL, C.POINTER(C.c_ubyte)]
         L.oracle_get_prims.argtypes = [C.c_void_p, _DBL]
+        L.oracle_stats_accumulate.argtypes = [C.c_void_p]
+        L.oracle_stats_read.argtypes = [C.c_void_p, _DBL, C.POINTER(C.c_longlong)]
+        L.oracle_stats_reset.argtypes = [C.c_void_p]
         L.oracle_get_ghosted.argtypes = [C.c_void_p, _DBL]
         L.oracle_roe_state.argtypes = [C.c_double, _DBL, C.c_double, C.c_double, _DBL, C.c_double, _DBL, _DBL]
         L.oracle_roe_state.restype = None
@@ -204,6 +207,19 @@ class Oracle:
         fl = np.empty((3,) + self.shape[1:], dtype=np.uint8)
         self._chk(lib().oracle_get_sensor(self._h, _p(th), fl.ctypes.data_as(C.POINTER(C.c_ubyte))))
         return th, fl
+
+    def stats_accumulate(self):
+        self._chk(lib().oracle_stats_accumulate(self._h))
+
+    def stats_read(self):
+        """(profiles [16][ny], number of samples): rho,u,v,w,p,T,mu,rho u,rho v,rho w,rho T,rho uu,rho vv,rho ww,rho uv,TT"""
+        out = np.empty((16, self.n[1]))
+        n = C.c_longlong(0)
+        self._chk(lib().oracle_stats_read(self._h, _p(out), C.byref(n)))
+        return out, n.value
+
+    def stats_reset(self):
+        self._chk(lib().oracle_stats_reset(self._h))
 
     def ghosted(self):
         """Ghost-filled conservative state [5][nz+6][ny+6][nx+6] (S1)."""

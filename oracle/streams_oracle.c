@@ -61,6 +61,8 @@ struct oracle_ctx {
   double* Rprev;   /* R of the previous RK stage                       */
   double* Rcur;
   double post[5];  /* shock generator post-shock primitive state       */
+  double* stat_sum;  /* [ORC_NSTAT][ny] running sums of the plane means (statistics) */
+  long long stat_n;
   int has_state;
   long long step;
   double time, dt, force;
@@ -259,6 +261,7 @@ int oracle_create(const oracle_grid* g, const double* x, const double* y, const 
   c->inflow = (double*)calloc((size_t)NV * c->n[1] * c->n[2], sizeof(double));
   c->Rprev = (double*)calloc(NV * c->np, sizeof(double));
   c->Rcur = (double*)calloc(NV * c->np, sizeof(double));
+  c->stat_sum = (double*)calloc((size_t)ORC_NSTAT * c->n[1], sizeof(double));
   *out = c;
   return ORC_OK;
 }
@@ -266,7 +269,7 @@ int oracle_create(const oracle_grid* g, const double* x, const double* y, const 
 void oracle_destroy(oracle_ctx* c) {
   if (!c) return;
   for (int d = 0; d < 3; ++d) { free(c->xc[d]); free(c->h[d]); free(c->gm[d]); free(c->dd[d]); }
-  free(c->w); free(c->wg); free(c->q); free(c->theta); free(c->inflow); free(c->Rprev); free(c->Rcur);
+  free(c->w); free(c->wg); free(c->q); free(c->theta); free(c->inflow); free(c->Rprev); free(c->Rcur); free(c->stat_sum);
   free(c);
 }
 
@@ -853,6 +856,53 @@ int oracle_step(oracle_ctx* c, int nsteps) {
     c->time += dt;
     c->step += 1;
   }
+  return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* Statistics: "the overline symbol denotes averaging in the homogeneous space directions and in
+ * time"; Reynolds means of phi and the density-weighted sums that give Favre means  phi~ = mean(rho phi) / mean(rho).
+ * One call adds the x-z plane means (plain node means: the homogeneous directions are uniformly spaced) of the
+ * current state to running sums, per wall-normal index j.  Order of the ORC_NSTAT quantities:
+ *   rho, u, v, w, p, T, mu, rho u, rho v, rho w, rho T, rho u u, rho v v, rho w w, rho u v, T T                  */
+int oracle_stats_accumulate(oracle_ctx* c) {
+  if (!c) return ORC_EINVAL;
+  if (!c->has_state) return ORC_ESTATE;
+  fill_ghosts(c);
+  compute_prims(c);
+  const size_t NP = c->NP;
+  const double cnt = (double)c->n[0] * (double)c->n[2];
+  for (int j = 0; j < c->n[1]; ++j) {
+    ksum acc[ORC_NSTAT];
+    for (int m = 0; m < ORC_NSTAT; ++m) { acc[m].s = 0.0; acc[m].c = 0.0; }
+    for (int k = 0; k < c->n[2]; ++k)
+      for (int i = 0; i < c->n[0]; ++i) {
+        const size_t o = GI(c, i, j, k);
+        const double rho = c->q[Q_RHO * NP + o], u = c->q[Q_U * NP + o], v = c->q[Q_V * NP + o], w = c->q[Q_W * NP + o];
+        const double pr = c->q[Q_P * NP + o], T = c->q[Q_T * NP + o], mu = c->q[Q_MU * NP + o];
+        const double val[ORC_NSTAT] = {rho, u, v, w, pr, T, mu, rho * u, rho * v, rho * w, rho * T,
+                                       rho * u * u, rho * v * v, rho * w * w, rho * u * v, T * T};
+        for (int m = 0; m < ORC_NSTAT; ++m) kadd(&acc[m], val[m]);
+      }
+    for (int m = 0; m < ORC_NSTAT; ++m) c->stat_sum[(size_t)m * c->n[1] + j] += (acc[m].s + acc[m].c) / cnt;
+  }
+  c->stat_n += 1;
+  return ORC_OK;
+}
+
+/* time-averaged profiles [ORC_NSTAT][ny] = running sums / number of accumulated samples */
+int oracle_stats_read(oracle_ctx* c, double* out, long long* nsamples) {
+  if (!c || !out) return ORC_EINVAL;
+  const double inv = c->stat_n > 0 ? 1.0 / (double)c->stat_n : 0.0;
+  for (size_t e = 0; e < (size_t)ORC_NSTAT * c->n[1]; ++e) out[e] = c->stat_sum[e] * inv;
+  if (nsamples) *nsamples = c->stat_n;
+  return ORC_OK;
+}
+
+int oracle_stats_reset(oracle_ctx* c) {
+  if (!c) return ORC_EINVAL;
+  memset(c->stat_sum, 0, (size_t)ORC_NSTAT * c->n[1] * sizeof(double));
+  c->stat_n = 0;
   return ORC_OK;
 }
 

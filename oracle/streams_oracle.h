@@ -21,6 +21,7 @@ enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENONFINITE = -4, ORC_ESTATE = -5 };
 enum { ORC_BC_PERIODIC = 0, ORC_BC_WALL_STAG = 1, ORC_BC_WALL_NODE = 2, ORC_BC_INFLOW = 3,
        ORC_BC_OUTFLOW = 4, ORC_BC_SHOCKGEN = 5, ORC_BC_EXTRAP = 6 };
 enum { ORC_VISC_POWER = 0, ORC_VISC_SUTHERLAND = 1 };
+enum { ORC_NSTAT = 16 };   /* statistics per wall-normal index, see oracle_stats_accumulate */
 
 typedef struct { int nx, ny, nz; int pad_; double len[3]; } oracle_grid;
 
@@ -55,6 +56,10 @@ int  oracle_step(oracle_ctx*, int nsteps);
 int  oracle_diagnostics(oracle_ctx*, oracle_diag* out);
 void oracle_destroy(oracle_ctx*);
 int  oracle_threads(void);
+/* Reynolds / Favre statistics: plane means over the homogeneous directions x, z, averaged over calls */
+int  oracle_stats_accumulate(oracle_ctx*);
+int  oracle_stats_read(oracle_ctx*, double* out /* [ORC_NSTAT][ny] */, long long* nsamples);
+int  oracle_stats_reset(oracle_ctx*);
 
 /* pieces exposed so that tests can pin them one by one */
 int  oracle_coeffs(int order, double a_out[3], double b_out[3]);            /* a_l, b_l tables        */

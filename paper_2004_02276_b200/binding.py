@@ -16,7 +16,7 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, S
 
 EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
-           "streams_diagnostics", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
+           "streams_diagnostics", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
 
 
 class StreamsGrid(C.Structure):
@@ -72,6 +72,9 @@ def lib():
         L.streams_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.streams_step.argtypes = [C.c_void_p, C.c_int]
         L.streams_diagnostics.argtypes = [C.c_void_p, C.POINTER(StreamsDiag)]
+        L.streams_stats_accumulate.argtypes = [C.c_void_p]
+        L.streams_stats_read.argtypes = [C.c_void_p, _DBL, C.POINTER(C.c_longlong)]
+        L.streams_stats_reset.argtypes = [C.c_void_p]
         L.streams_profile.argtypes = [C.c_void_p, C.c_int]
         L.streams_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.streams_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
@@ -140,7 +143,10 @@ class Streams:
             raise StreamsError(STREAMS_EINVAL, "invalid grid/params")
         with torch.cuda.device(self.device):
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            # a private (non-blocking) stream per context: the library's launches do not serialise with the legacy
+            # default stream, and streams_step may capture its kernels into CUDA graphs (include/streams.h).  A
+            # caller-supplied torch stream is used as given (the legacy default stream disables the graphs).
+            self._stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
             xs = [np.ascontiguousarray(a, dtype=np.float64) for a in (x, y, z)]
             h = C.c_void_p()
             rc = lib().streams_create(C.byref(self._g), xs[0].ctypes.data_as(_DBL), xs[1].ctypes.data_as(_DBL),
@@ -163,6 +169,27 @@ class Streams:
         except Exception:
             pass
 
+    @property
+    def stream(self):
+        """The torch.cuda.Stream all kernels of this context are enqueued on."""
+        return self._stream
+
+    def _pre(self, t=None):
+        """The context stream waits for what the caller's current stream has enqueued (producer of `t`)."""
+        cur = self._torch.cuda.current_stream(self.device)
+        if cur != self._stream:
+            self._stream.wait_stream(cur)
+            if t is not None:
+                t.record_stream(self._stream)
+
+    def _post(self, t=None):
+        """The caller's current stream waits for the context stream (consumer of `t`)."""
+        cur = self._torch.cuda.current_stream(self.device)
+        if cur != self._stream:
+            cur.wait_stream(self._stream)
+            if t is not None:
+                t.record_stream(self._stream)
+
     def _chk(self, rc, allow=()):
         if rc != 0 and rc not in allow:
             raise StreamsError(rc, lib().streams_last_error(self._h).decode())
@@ -184,6 +211,7 @@ class Streams:
             assert w.shape == self.shape
             self._chk(lib().streams_set_state_host(self._h, C.c_void_p(w.ctypes.data)))
         else:
+            self._pre(w)
             self._chk(lib().streams_set_state(self._h, self._dev(w, self.shape)))
 
     def set_state_host_ptr(self, ptr):
@@ -196,7 +224,9 @@ class Streams:
         torch = self._torch
         if out is None:
             out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._pre()
         self._chk(lib().streams_get_state(self._h, self._dev(out, self.shape)))
+        self._post(out)
         return out
 
     def get_state_host(self):
@@ -209,14 +239,19 @@ class Streams:
         torch = self._torch
         if out is None:
             out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._pre()
         self._chk(lib().streams_rhs(self._h, self._dev(out, self.shape)))
+        self._post(out)
         return out
 
     def sensor(self):
         torch = self._torch
         th = torch.empty(self.shape[1:], dtype=torch.float64, device=self.device)
         fl = torch.empty((3,) + self.shape[1:], dtype=torch.uint8, device=self.device)
+        self._pre()
         self._chk(lib().streams_sensor(self._h, C.c_void_p(th.data_ptr()), C.c_void_p(fl.data_ptr())))
+        self._post(th)
+        self._post(fl)
         return th, fl
 
     def step(self, n=1):
@@ -227,6 +262,20 @@ class Streams:
         rc = lib().streams_diagnostics(self._h, C.byref(d))
         self._chk(rc, allow=() if check else (STREAMS_ENONFINITE,))
         return d
+
+    # --- statistics --------------------------------------------------------------
+    def stats_accumulate(self):
+        self._chk(lib().streams_stats_accumulate(self._h))
+
+    def stats_read(self):
+        """(time-averaged x-z plane means [16][ny] as a NumPy array, number of samples)"""
+        out = np.empty((16, self.n[1]))
+        n = C.c_longlong(0)
+        self._chk(lib().streams_stats_read(self._h, out.ctypes.data_as(_DBL), C.byref(n)))
+        return out, n.value
+
+    def stats_reset(self):
+        self._chk(lib().streams_stats_reset(self._h))
 
     def profile(self, enable=True):
         self._chk(lib().streams_profile(self._h, 1 if enable else 0))

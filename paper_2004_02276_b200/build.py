@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libstreams_b200.so")
 SOURCES = ["streams.cu"]
-DEPS = ["streams.cu", "dev_common.cuh", "k_rhs.cuh", "k_aux.cuh", "k_weno.cuh"]
+DEPS = ["streams.cu", "dev_common.cuh", "k_rhs.cuh", "k_aux.cuh", "k_weno.cuh", "k_stats.cuh"]
 
 
 def _stale() -> bool:

@@ -57,7 +57,7 @@ constexpr int SM_GRING = 7 * 3 * NPT;
 constexpr int SM_RRING = 3 * 5 * NPT;     // R of planes s-1..s-3: read (plane s-3) before written (plane s) in a step
 constexpr int NOWN = 3;                         // own-node ring: plane s+3 is read while s+4, s+5 are in flight
 constexpr int SM_OWN = NOWN * NF * NPT;
-constexpr int SM_SPREV = 6 * NPT;                // FUSED: R_prev (5) and u_prev of plane s-3, prefetched by cp.async
+constexpr int SM_SPREV = 2 * 6 * NPT;            // FUSED: R_prev (5) and u_prev of planes s-3 / s-2, prefetched by cp.async one step ahead
 constexpr int SM_PCOPY = (sizeof(DevP) + 7) / 8;   // copy of the parameter block for the out-of-line helpers
 constexpr int SM_RED = 32;
 constexpr int LZ_MAX = 128;                     // planes per CTA (make_layout caps the chunk length)
@@ -391,7 +391,6 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
   const bool edge = !use_tma || i0 < HALO || i0 + TX + HALO > P.nx || j0 < HALO || j0 + TY + HALO > P.ny;
   const int nplanes = k1 + 3 - (k0 - 3);
-  constexpr bool zfirst = false;                         // (phase stagger between warp halves: measured +1 %, costs a second copy of the z block)
 
   if (tid == 0) {
     *pcount = 0;
@@ -482,16 +481,18 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 #pragma unroll
       for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.N);
     }
-    if (FUSED && A.alpha != 0.0 && active && s - 3 >= k0) {
-      // R_prev (and u_prev for the lazy forcing) of plane s-3, read in this step's epilogue
-      const size_t o = (size_t)(s - 3) * P.nxy + own_off;
-      const unsigned d = smem_u32(spring + tid);
+    if (FUSED && A.alpha != 0.0 && active && s - 2 >= k0 && s - 2 < k1) {
+      // R_prev (and u_prev for the lazy forcing) of plane s-2, read in the NEXT step's epilogue (one step of slack:
+      // the epilogue sits before the plane barrier and must not wait for HBM)
+      const size_t o = (size_t)(s - 2) * P.nxy + own_off;
+      const unsigned d = smem_u32(spring + tid) + (((it + 1) & 1) * 6 * NPT) * 8;
 #pragma unroll
       for (int v = 0; v < 5; ++v) cp_async8(d + v * NPT * 8, A.S_prev + o + v * P.N);
       if (A.f_prev) cp_async8(d + 5 * NPT * 8, A.q_out + o + P.N);
     }
     cp_async_commit();
-    cp_async_wait<2>();                                  // plane s+3 has landed (requested at step s-2)
+    cp_async_wait<1>();                                  // the groups of steps <= s-1 have landed: own node of plane s+3
+                                                         // (and s+4), R_prev of plane s-3
     int tl = tid;                                        // opaque copy: keeps per-thread shared-memory addresses from being
     asm volatile("" : "+r"(tl));                         // hoisted out of the loop (and then spilled) instead of recomputed
     const int li = tl & (TX - 1), lj = tl / TX, loc = (lj + HALO) * PITCH + li + XH;
@@ -500,6 +501,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     // lower half after arriving at the barrier, so that the two warps of a scheduler are in different phases
     // (fp64-dense z against the shared-memory-heavy x, y)
     NodeAcc N;
+    Nb o3;                                               // own node of plane s+3: read ONCE (l = 3 pair, then the window)
     auto zdir = [&]() {
       Nb c;
       c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
@@ -511,8 +513,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         if (l < 3) {
           p.rho = rw[3 + l]; p.u = uw[3 + l]; p.v = vw[3 + l]; p.w = ww[3 + l]; p.T = Tw[3 + l]; p.mu = mw[3 + l]; p.H = Hw[3 + l];
         } else {
-          p.rho = own3[F_RHO * NPT]; p.u = own3[F_U * NPT]; p.v = own3[F_V * NPT]; p.w = own3[F_W * NPT];
-          p.T = own3[F_T * NPT]; p.mu = own3[F_MU * NPT]; p.H = own3[F_H * NPT];
+          p = o3;
         }
         m.rho = rw[3 - l]; m.u = uw[3 - l]; m.v = vw[3 - l]; m.w = ww[3 - l]; m.T = Tw[3 - l]; m.mu = mw[3 - l]; m.H = Hw[3 - l];
         dir_accum<2>(P.c.a[l - 1], P.c.b[l - 1], P.c.qa[l - 1], P.c.aR[l - 1], c, p, m, Z);
@@ -525,7 +526,6 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 #pragma unroll
       for (int v = 0; v < 5; ++v) N.R[v] = 0.0;
       N.Va[0] = N.Va[1] = N.Va[2] = 0.0; N.LT = 0.0; N.heat = 0.0;
-      if (zfirst) zdir();
     }
     if (use_tma) mbar_wait(bar0 + 8 * buf, phase);
     if (edge && it + 1 < nplanes) {
@@ -613,22 +613,32 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     __syncwarp();
     if ((tl & 31) == 0) mbar_arrive(sbar);
 
-    if (!zfirst && active && full) zdir();
-    // ---- second half of the barrier: the staging rows of this plane are complete ----
-    mbar_wait(sbar, (unsigned)(it & 1));
-    if (FUSED) cp_async_wait<0>();                       // R_prev / u_prev of plane s-3 (requested at the top of the step)
-    // every thread is past its reads of this plane's tile: the buffer takes plane s+2
-    if (use_tma && tl == 0 && it + 2 < nplanes) {
-      const int b2 = buf;                                // (it + 2) % NBUF
-      fence_proxy_async();
-      mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
-      tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
-    }
-    // ================= after the barrier: plane p = s-3 is completed and written (z-mixed terms, epilogue), plane s
-    // is assembled (xy mixed terms, viscous stresses) into the residual ring.  The two are independent dependency
-    // chains; on plain tiles in the interior of a chunk they sit in ONE straight block so that they interleave.
+    // ================= between arrive and wait: everything that needs no other thread's data of this plane.  The z
+    // direction, the viscous assembly of plane s without its xy mixed terms, and the completion + epilogue of plane
+    // p = s-3 (z-mixed terms from the thread-private rings, Eq. 11, global stores) -- more than half of the step's
+    // work, so that the wait below finds the barrier complete (measured: the wait was 6 % of all warp cycles when it
+    // sat directly after the z direction).
+    o3.rho = own3[F_RHO * NPT]; o3.u = own3[F_U * NPT]; o3.v = own3[F_V * NPT]; o3.w = own3[F_W * NPT];
+    o3.T = own3[F_T * NPT]; o3.mu = own3[F_MU * NPT]; o3.H = own3[F_H * NPT];
     const int p = s - 3;
-    auto finish_p = [&]() {
+    const bool do_fin = active && p >= k0, do_asm = active && full;
+    if (do_asm) {
+      zdir();
+      if (A.nflag) {
+        // S4 / Eq. 8 (PAPER.md:81): same expression, same order as k_sensor (the flags must agree bit for bit)
+        const double* G = N.G;
+        const double div = G[0] + G[4] + G[8];
+        const double ox = G[7] - G[5], oy = G[2] - G[6], oz = G[3] - G[1];
+        const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
+        A.nflag[(size_t)s * P.nxy + own_off] = th > P.th_thr ? 1 : 0;
+      }
+      if (PLAIN || P.viscous) {
+        Nb c;
+        c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
+        visc_assemble(P, c, N);                          // N.R is final up to the xy mixed terms (added after the wait)
+      }
+    }
+    if (do_fin) {
       double R[5];
       {
         const double* rr = rring + b3 * 5 * NPT + tl;               // plane s-3 sits in slot it % 3
@@ -662,7 +672,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       } else {
         double dW[5];
         const double dt = scal[0], fprev = scal[1];
-        const double* pv = spring + tl;
+        const double* pv = spring + (it & 1) * 6 * NPT + tl;        // requested at the top of step s-1
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
           double sp = A.alpha != 0.0 ? pv[v * NPT] : 0.0;
@@ -680,10 +690,21 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 6 * P.N] = qn.H;
         if (store_mu) A.q_out[o + 5 * P.N] = qn.mu;
       }
-        };
-    auto assemble_s = [&]() {
+    }
+    // ---- second half of the barrier: the staging rows of this plane are complete ----
+    mbar_wait(sbar, (unsigned)(it & 1));
+    // every thread is past its reads of this plane's tile: the buffer takes plane s+2
+    if (use_tma && tl == 0 && it + 2 < nplanes) {
+      const int b2 = buf;                                // (it + 2) % NBUF
+      fence_proxy_async();
+      mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
+      tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
+    }
+    // ================= after the barrier: the xy mixed terms of plane s (A8), d_x(d_y v) and d_y(d_x u) from the
+    // staging rows; they enter V_0, V_1 times mu / 3 and the viscous work u V_0 + v V_1.  R of plane s goes to the
+    // residual ring (its slot was read above: plane s-3).
+    if (do_asm) {
       if (PLAIN || P.viscous) {
-        // xy mixed terms (A8): d_x(d_y v) and d_y(d_x u) from the staging rows
         const int sy = lj * PITCH + li + XH, sx = (lj + HALO) * TX + li;
         double mxy = P.c.a[0] * (sgY[sy + 1] - sgY[sy - 1]);
         mxy = fma(P.c.a[1], sgY[sy + 2] - sgY[sy - 2], mxy);
@@ -691,34 +712,14 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         double myx = P.c.a[0] * (sgX[sx + TX] - sgX[sx - TX]);
         myx = fma(P.c.a[1], sgX[sx + 2 * TX] - sgX[sx - 2 * TX], myx);
         myx = fma(P.c.a[2], sgX[sx + 3 * TX] - sgX[sx - 3 * TX], myx);
-        const double ixy3 = xi[li] * yi[lj] * (1.0 / 3.0);
-        N.Va[0] = fma(mxy, ixy3, N.Va[0]);
-        N.Va[1] = fma(myx, ixy3, N.Va[1]);
-        Nb c;
-        c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
-        visc_assemble(P, c, N);
+        const double m3 = mw[3] * (xi[li] * yi[lj] * (1.0 / 3.0));
+        const double v0 = m3 * mxy, v1 = m3 * myx;
+        N.R[1] += v0; N.R[2] += v1;
+        N.R[4] += fma(uw[3], v0, vw[3] * v1);
       }
       double* rr = rring + b3 * 5 * NPT + tl;
 #pragma unroll
       for (int v = 0; v < 5; ++v) rr[v * NPT] = N.R[v];
-        };
-    const bool do_fin = active && p >= k0, do_asm = active && full;
-    if (PLAIN && do_fin && do_asm) {
-      finish_p();
-      assemble_s();
-    } else {
-      if (do_fin) finish_p();
-      if (do_asm) assemble_s();
-    }
-    if (do_asm) {
-      if (A.nflag) {
-        // S4 / Eq. 8 (PAPER.md:81): same expression, same order as k_sensor (the flags must agree bit for bit)
-        const double* G = N.G;
-        const double div = G[0] + G[4] + G[8];
-        const double ox = G[7] - G[5], oy = G[2] - G[6], oz = G[3] - G[1];
-        const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
-        A.nflag[(size_t)s * P.nxy + own_off] = th > P.th_thr ? 1 : 0;
-      }
     }
     slot7 = slot7 == 6 ? 0 : slot7 + 1;
     b3 = b3 == 2 ? 0 : b3 + 1;
@@ -728,8 +729,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       rw[a] = rw[a + 1]; uw[a] = uw[a + 1]; vw[a] = vw[a + 1]; ww[a] = ww[a + 1]; Tw[a] = Tw[a + 1]; mw[a] = mw[a + 1]; Hw[a] = Hw[a + 1];
     }
     if (active && s + 3 < k1 + 3) {
-      rw[5] = own3[F_RHO * NPT]; uw[5] = own3[F_U * NPT]; vw[5] = own3[F_V * NPT]; ww[5] = own3[F_W * NPT];
-      Tw[5] = own3[F_T * NPT]; mw[5] = own3[F_MU * NPT]; Hw[5] = own3[F_H * NPT];
+      rw[5] = o3.rho; uw[5] = o3.u; vw[5] = o3.v; ww[5] = o3.w; Tw[5] = o3.T; mw[5] = o3.mu; Hw[5] = o3.H;
     }
   }
   if (A.partial) {

@@ -15,6 +15,7 @@
 #include "dev_common.cuh"
 #include "k_aux.cuh"
 #include "k_rhs.cuh"
+#include "k_stats.cuh"
 #include "k_weno.cuh"
 
 using namespace streams;
@@ -54,6 +55,17 @@ struct streams_ctx {
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
   int prof_on, prof_n;
   std::vector<cudaEvent_t>* prof_ev;   // pairs (start, stop) around k_rhs
+  int device;                          // CUDA device the context was created on; every entry point switches to it
+  // one RK3 step as a CUDA graph (launch-bound small grids): one executable per host-state key, see step_key()
+  int graph_ok;                        // 0: direct launches only (legacy default stream, capture failed, disabled)
+  cudaGraphExec_t gexec[8];
+  int g_after[8];                      // host state (key) after the step captured from key k
+  int g_launches[8];                   // kernel launches inside the graph (bench accounting)
+  double* stat_partial;                // [STAT_ZC][NSTAT][ny] chunk sums of the statistics pass (context-owned, O(ny))
+  double* stat_sum;                    // [NSTAT][ny] running sums of the plane means
+  unsigned long long* stat_n;          // accumulated samples
+  DevScal* h_sc;                       // pinned host copies for streams_diagnostics (no pageable-memory async copies)
+  double* h_part;
   char err[256];
 };
 
@@ -81,6 +93,13 @@ int cuda_fail(streams_ctx* c, cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(c, e_, name);          \
   } while (0)
 
+// every entry point runs on the device the context was created on, whatever the caller's current device is
+struct DevGuard {
+  int prev = -1, dev;
+  explicit DevGuard(int d) : dev(d) { if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) cudaSetDevice(dev); else prev = dev; }
+  ~DevGuard() { if (prev != dev) cudaSetDevice(prev); }
+};
+
 bool coeffs(int order, Coef& k) {
   for (int i = 0; i < 3; ++i) k.a[i] = k.b[i] = k.qa[i] = k.aR[i] = 0.0;
   k.sb2 = 0.0;
@@ -94,6 +113,7 @@ const char* validate(const streams_grid* g, const streams_params* p) {
   if (g->nx < 1 || g->ny < 1 || g->nz < 1) return "grid sizes must be >= 1";
   if ((long long)g->nx * g->ny * g->nz > 0xffffffffLL) return "more than 2^32 nodes";
   if ((long long)g->nx * g->ny > 0x3fffffffLL) return "more than 2^30 nodes per z-plane";
+  if ((long long)g->ny * g->nz > 0x7fffffffLL) return "more than 2^31 grid rows (ny * nz)";
   if (!(p->gamma > 1.0) || !(p->Rgas > 0.0) || !(p->Pr > 0.0)) return "gamma > 1, Rgas > 0, Pr > 0 required";
   if (p->order != 2 && p->order != 4 && p->order != 6) return "order must be 2, 4 or 6";
   if (p->weno_enable && (long long)g->nx * g->ny * g->nz > 0x7fffffffLL) return "more than 2^31 nodes with the hybrid switch on (interface lists)";
@@ -280,7 +300,11 @@ int streams_fp64_peak(void* cuda_stream, double* h_tinstr) {
 
 void streams_destroy(streams_ctx* c) {
   if (!c) return;
+  DevGuard dg(c->device);
   cudaStreamSynchronize(c->st);
+  for (int k = 0; k < 8; ++k) if (c->gexec[k]) cudaGraphExecDestroy(c->gexec[k]);
+  if (c->h_sc) cudaFreeHost(c->h_sc);
+  if (c->h_part) cudaFreeHost(c->h_part);
   if (c->small_dev) cudaFree(c->small_dev);
   if (c->prof_ev) { for (cudaEvent_t e : *c->prof_ev) cudaEventDestroy(e); delete c->prof_ev; }
   delete c;
@@ -288,6 +312,7 @@ void streams_destroy(streams_ctx* c) {
 
 int streams_profile(streams_ctx* c, int enable) {
   if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   if (enable && !c->prof_ev) {
     c->prof_ev = new std::vector<cudaEvent_t>(2 * 4096);
     for (cudaEvent_t& e : *c->prof_ev) CK(cudaEventCreate(&e));
@@ -299,6 +324,7 @@ int streams_profile(streams_ctx* c, int enable) {
 
 int streams_profile_read(streams_ctx* c, double* ms_total, long long* launches) {
   if (!c || !ms_total || !launches) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   CK(cudaStreamSynchronize(c->st));
   double tot = 0.0;
   for (int i = 0; i < c->prof_n; ++i) {
@@ -327,6 +353,9 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   snprintf(c->err, sizeof c->err, "no error");
   c->g = *g; c->p = *p;
   c->st = (cudaStream_t)cuda_stream;
+  if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return fail(nullptr, STREAMS_ECUDA, "cudaGetDevice failed"); }
+  // stream capture is not allowed on the legacy default stream: graphs need a stream of the caller's own
+  c->graph_ok = (c->st != nullptr && c->st != cudaStreamLegacy && c->st != cudaStreamPerThread) ? 1 : 0;
   char* base = (char*)d_workspace;
   for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]); c->S[i] = (double*)(base + L.S[i]); }
   if (p->weno_enable) {
@@ -409,10 +438,11 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   }
 
   // ---- small device arrays ----
-  size_t off = 0, o_arr[9], o_xpost, o_sc;
+  size_t off = 0, o_arr[9], o_xpost, o_sc, o_stat;
   for (int a = 0; a < 9; ++a) { o_arr[a] = off; off += up((size_t)n[a % 3] * sizeof(double)); }
   o_xpost = off; off += up(xpost.size());
   o_sc = off; off += up(sizeof(DevScal));
+  o_stat = off; off += up(((size_t)(STAT_ZC + 1) * NSTAT * n[1] + 1) * sizeof(double));
   cudaError_t e = cudaMalloc(&c->small_dev, off);
   if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(metrics)"); }
   char* sb = (char*)c->small_dev;
@@ -426,6 +456,10 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   P.xpost = (const unsigned char*)(sb + o_xpost);
   P.inflow = c->inflow;
   c->sc = (DevScal*)(sb + o_sc);
+  c->stat_partial = (double*)(sb + o_stat);
+  c->stat_sum = c->stat_partial + (size_t)STAT_ZC * NSTAT * n[1];
+  c->stat_n = (unsigned long long*)(c->stat_sum + (size_t)NSTAT * n[1]);
+  cudaMemsetAsync(c->stat_sum, 0, ((size_t)NSTAT * n[1] + 1) * sizeof(double), c->st);
   DevScal hs;
   std::memset(&hs, 0, sizeof hs);
   hs.vol_total = voltot;
@@ -442,6 +476,9 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
         cudaFree(c->small_dev); delete c;
         return fail(nullptr, STREAMS_ECUDA, "cuTensorMapEncodeTiled failed");
       }
+  e = cudaMallocHost((void**)&c->h_sc, sizeof(DevScal));
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_part, ((size_t)NDIAG * RGRID + 8) * sizeof(double));
+  if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaMallocHost(diagnostics)"); }
   e = cudaFuncSetAttribute(k_rhs<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
@@ -469,10 +506,12 @@ static int after_set_state(streams_ctx* c, const double* d_w) {
 
 int streams_set_state(streams_ctx* c, const double* d_w) {
   if (!c || !d_w) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   return after_set_state(c, d_w);
 }
 int streams_set_state_host(streams_ctx* c, const double* h_w) {
   if (!c || !h_w) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   // the RK register S[1] is free between steps: it stages the conservative vector
   CK(cudaMemcpyAsync(c->S[1], h_w, 5 * (size_t)c->P.N * sizeof(double), cudaMemcpyHostToDevice, c->st));
   const int rc = after_set_state(c, c->S[1]);
@@ -482,6 +521,7 @@ int streams_set_state_host(streams_ctx* c, const double* h_w) {
 }
 int streams_get_state(streams_ctx* c, double* d_w) {
   if (!c || !d_w) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   k_prim2cons<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->qbuf[c->cur], d_w);
   LAUNCH_CHECK("k_prim2cons");
@@ -489,6 +529,7 @@ int streams_get_state(streams_ctx* c, double* d_w) {
 }
 int streams_get_state_host(streams_ctx* c, double* h_w) {
   if (!c || !h_w) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   k_prim2cons<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->S[1]);
   LAUNCH_CHECK("k_prim2cons");
@@ -563,6 +604,7 @@ static int force_from_partials(streams_ctx* c, const double* R, bool have_rhs_pa
 
 int streams_rhs(streams_ctx* c, double* d_rhs) {
   if (!c || !d_rhs) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   const double* w = c->qbuf[c->cur];
   int rc;
@@ -585,86 +627,165 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
 
 int streams_sensor(streams_ctx* c, double* d_theta, unsigned char* d_flags) {
   if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   if (!c->p.weno_enable) return fail(c, STREAMS_EINVAL, "streams_sensor needs weno_enable = 1");
   return run_sensor(c, c->qbuf[c->cur], d_theta, d_flags, false);
 }
 
-int streams_step(streams_ctx* c, int nsteps) {
-  if (!c || nsteps < 0) return fail(c, STREAMS_EINVAL, "bad argument");
-  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+// host state that decides which kernels one RK3 step launches and on which buffers
+static int step_key(const streams_ctx* c) { return c->cur | (c->scur << 1) | (c->dt_ready << 2); }
+
+// enqueue ONE RK3 step (Eq. 11) on the context stream and advance the host-side state (buffers, dt_ready)
+static int step_once(streams_ctx* c) {
   static const double alpha[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};   // Eq. 11 with the sign of reading G5
   static const double beta[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
   const int rg = rgrid_for(c->P.N);
   int rc;
-  for (int s = 0; s < nsteps; ++s) {
-    if (!(c->p.dt_fixed > 0.0) && c->dt_ready) {
-      k_take_dt<<<1, 1, 0, c->st>>>(c->sc);
-      LAUNCH_CHECK("k_take_dt");
-      c->dt_ready = 0;
-    } else if (!(c->p.dt_fixed > 0.0)) {
-      k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->partial);
-      LAUNCH_CHECK("k_speed_partial");
-      k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 1);
-      LAUNCH_CHECK("k_dt_final");
-    }
-    for (int l = 0; l < 3; ++l) {
-      double* w = c->qbuf[c->cur];
-      RhsArgs A;
-      std::memset(&A, 0, sizeof A);
-      A.q = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
-      if (c->p.forcing && !c->p.weno_enable) {
-        // lazy forcing: the fused kernel advances with alpha (R_prev + f_prev ...) + beta R and sums R_rhou; once f is
-        // known a light kernel adds dt beta f (e_rhou + u e_rhoE).  S[0] keeps R without the forcing terms.
-        double* wn = c->qbuf[c->cur ^ 1];
-        A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
-        A.f_prev = l > 0 ? &c->sc->force : nullptr;
-        A.write_S = l < 2 ? 1 : 0;
-        if ((rc = launch_rhs(c, 2, A))) return rc;
-        if ((rc = force_from_partials(c, nullptr, true))) return rc;
-        const bool want_dt = l == 2 && !(c->p.dt_fixed > 0.0);
-        k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l], want_dt ? c->partial : nullptr);
-        LAUNCH_CHECK("k_force_fix");
-        if (want_dt) {
-          k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 2);
-          LAUNCH_CHECK("k_dt_final");
-          c->dt_ready = 1;
-        }
-        c->cur ^= 1;
-      } else if (c->p.forcing) {
-        // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
-        double* Sp = c->S[c->scur];
-        double* Sc = c->S[c->scur ^ 1];
-        const bool partial_ok = !c->p.weno_enable;
-        A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
-        if ((rc = launch_rhs(c, 0, A))) return rc;
-        if (c->p.weno_enable) {
-          if ((rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
-        }
-        if ((rc = force_from_partials(c, Sc, partial_ok))) return rc;
-        k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1, l < 2 ? 1 : 0);
-        LAUNCH_CHECK("k_update");
-        c->scur ^= 1;
-      } else {
-        // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
-        double* wn = c->qbuf[c->cur ^ 1];
-        A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
-        if ((rc = launch_rhs(c, 1, A))) return rc;
-        if (c->p.weno_enable) {
-          if ((rc = run_weno(c, w, c->S[0], wn, beta[l]))) return rc;
-        }
-        c->cur ^= 1;
+  if (!(c->p.dt_fixed > 0.0) && c->dt_ready) {
+    k_take_dt<<<1, 1, 0, c->st>>>(c->sc);
+    LAUNCH_CHECK("k_take_dt");
+    c->dt_ready = 0;
+  } else if (!(c->p.dt_fixed > 0.0)) {
+    k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->partial);
+    LAUNCH_CHECK("k_speed_partial");
+    k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 1);
+    LAUNCH_CHECK("k_dt_final");
+  }
+  for (int l = 0; l < 3; ++l) {
+    double* w = c->qbuf[c->cur];
+    RhsArgs A;
+    std::memset(&A, 0, sizeof A);
+    A.q = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
+    if (c->p.forcing && !c->p.weno_enable) {
+      // lazy forcing: the fused kernel advances with alpha (R_prev + f_prev ...) + beta R and sums R_rhou; once f is
+      // known a light kernel adds dt beta f (e_rhou + u e_rhoE).  S[0] keeps R without the forcing terms.
+      double* wn = c->qbuf[c->cur ^ 1];
+      A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
+      A.f_prev = l > 0 ? &c->sc->force : nullptr;
+      A.write_S = l < 2 ? 1 : 0;
+      if ((rc = launch_rhs(c, 2, A))) return rc;
+      if ((rc = force_from_partials(c, nullptr, true))) return rc;
+      const bool want_dt = l == 2 && !(c->p.dt_fixed > 0.0);
+      k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l], want_dt ? c->partial : nullptr);
+      LAUNCH_CHECK("k_force_fix");
+      if (want_dt) {
+        k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 2);
+        LAUNCH_CHECK("k_dt_final");
+        c->dt_ready = 1;
       }
+      c->cur ^= 1;
+    } else if (c->p.forcing) {
+      // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
+      double* Sp = c->S[c->scur];
+      double* Sc = c->S[c->scur ^ 1];
+      const bool partial_ok = !c->p.weno_enable;
+      A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
+      if ((rc = launch_rhs(c, 0, A))) return rc;
+      if (c->p.weno_enable) {
+        if ((rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
+      }
+      if ((rc = force_from_partials(c, Sc, partial_ok))) return rc;
+      k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1, l < 2 ? 1 : 0);
+      LAUNCH_CHECK("k_update");
+      c->scur ^= 1;
+    } else {
+      // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
+      double* wn = c->qbuf[c->cur ^ 1];
+      A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
+      if ((rc = launch_rhs(c, 1, A))) return rc;
+      if (c->p.weno_enable) {
+        if ((rc = run_weno(c, w, c->S[0], wn, beta[l]))) return rc;
+      }
+      c->cur ^= 1;
     }
-    k_advance_time<<<1, 1, 0, c->st>>>(c->sc);
-    LAUNCH_CHECK("k_advance_time");
+  }
+  k_advance_time<<<1, 1, 0, c->st>>>(c->sc);
+  LAUNCH_CHECK("k_advance_time");
+  return STREAMS_OK;
+}
+
+// Small grids are launch-bound (config 1: 27 launches of a few microseconds per step): one RK3 step is captured into
+// a CUDA graph per host-state key and replayed.  Grids of >= GRAPH_MAX_POINTS launch directly (nothing to gain).
+constexpr long long GRAPH_MAX_POINTS = 1LL << 24;
+
+int streams_step(streams_ctx* c, int nsteps) {
+  if (!c || nsteps < 0) return fail(c, STREAMS_EINVAL, "bad argument");
+  DevGuard dg(c->device);
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  int rc;
+  for (int s = 0; s < nsteps; ++s) {
+    const bool graph = c->graph_ok && !c->prof_on && c->P.N < GRAPH_MAX_POINTS;
+    if (!graph) {
+      if ((rc = step_once(c))) return rc;
+      c->step++;
+      continue;
+    }
+    const int key = step_key(c);
+    if (!c->gexec[key]) {
+      // capture: the launches of step_once are recorded, not run; the host state it leaves is what a replay leaves
+      const int cur0 = c->cur, scur0 = c->scur, dtr0 = c->dt_ready;
+      const long long l0 = c->launches;
+      cudaGraph_t gph = nullptr;
+      cudaError_t e = cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal);
+      if (e != cudaSuccess) { c->graph_ok = 0; cudaGetLastError(); --s; continue; }
+      rc = step_once(c);
+      e = cudaStreamEndCapture(c->st, &gph);
+      const int after = step_key(c);
+      const int nl = (int)(c->launches - l0);
+      c->cur = cur0; c->scur = scur0; c->dt_ready = dtr0; c->launches = l0;
+      if (rc || e != cudaSuccess || !gph) { if (gph) cudaGraphDestroy(gph); c->graph_ok = 0; cudaGetLastError(); --s; continue; }
+      e = cudaGraphInstantiate(&c->gexec[key], gph, 0);
+      cudaGraphDestroy(gph);
+      if (e != cudaSuccess) { c->gexec[key] = nullptr; c->graph_ok = 0; cudaGetLastError(); --s; continue; }
+      c->g_after[key] = after; c->g_launches[key] = nl;
+    }
+    CK(cudaGraphLaunch(c->gexec[key], c->st));
+    const int after = c->g_after[key];
+    c->cur = after & 1; c->scur = (after >> 1) & 1; c->dt_ready = (after >> 2) & 1;
+    c->launches += c->g_launches[key];
     c->step++;
   }
   return STREAMS_OK;
 }
 
+int streams_stats_accumulate(streams_ctx* c) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  const int nzc = std::min(STAT_ZC, c->P.nz);
+  k_stats_partial<<<dim3(c->P.ny, nzc), RT, 0, c->st>>>(c->P, c->qbuf[c->cur], nzc, c->stat_partial);
+  LAUNCH_CHECK("k_stats_partial");
+  k_stats_final<<<(NSTAT * c->P.ny + 127) / 128, 128, 0, c->st>>>(c->P, c->stat_partial, nzc, c->stat_sum, c->stat_n);
+  LAUNCH_CHECK("k_stats_final");
+  return STREAMS_OK;
+}
+
+int streams_stats_read(streams_ctx* c, double* h_out, long long* h_nsamples) {
+  if (!c || !h_out) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
+  const size_t n = (size_t)NSTAT * c->P.ny;
+  std::vector<double> tmp(n + 1);
+  CK(cudaMemcpyAsync(tmp.data(), c->stat_sum, (n + 1) * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  CK(cudaStreamSynchronize(c->st));
+  unsigned long long cnt;
+  std::memcpy(&cnt, &tmp[n], sizeof cnt);
+  const double inv = cnt > 0 ? 1.0 / (double)cnt : 0.0;
+  for (size_t e = 0; e < n; ++e) h_out[e] = tmp[e] * inv;
+  if (h_nsamples) *h_nsamples = (long long)cnt;
+  return STREAMS_OK;
+}
+
+int streams_stats_reset(streams_ctx* c) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
+  CK(cudaMemsetAsync(c->stat_sum, 0, ((size_t)NSTAT * c->P.ny + 1) * sizeof(double), c->st));
+  return STREAMS_OK;
+}
+
 int streams_diagnostics(streams_ctx* c, streams_diag* out) {
   if (!c || !out) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   std::memset(out, 0, sizeof *out);
   const int rg = rgrid_for(c->P.N);
@@ -672,18 +793,18 @@ int streams_diagnostics(streams_ctx* c, streams_diag* out) {
   int rc;
   // sensor statistics of the current state (interface counts as the next RHS would see them)
   if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, false))) return rc;
-  DevScal hs;
-  CK(cudaMemcpyAsync(&hs, c->sc, sizeof hs, cudaMemcpyDeviceToHost, c->st));
+  DevScal& hs = *c->h_sc;
+  CK(cudaMemcpyAsync(c->h_sc, c->sc, sizeof hs, cudaMemcpyDeviceToHost, c->st));
   k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, w, c->partial);
   LAUNCH_CHECK("k_speed_partial");
   k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, c->speeds, 0);
   LAUNCH_CHECK("k_dt_final");
-  double sp[3];
-  CK(cudaMemcpyAsync(sp, c->speeds, sizeof sp, cudaMemcpyDeviceToHost, c->st));
+  double* sp = c->h_part + (size_t)NDIAG * RGRID;
+  CK(cudaMemcpyAsync(sp, c->speeds, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
   k_diag_partial<<<rg, RT, 0, c->st>>>(c->P, w, c->partial);
   LAUNCH_CHECK("k_diag_partial");
-  std::vector<double> part((size_t)NDIAG * rg);
-  CK(cudaMemcpyAsync(part.data(), c->partial, part.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+  double* part = c->h_part;
+  CK(cudaMemcpyAsync(part, c->partial, (size_t)NDIAG * rg * sizeof(double), cudaMemcpyDeviceToHost, c->st));
   CK(cudaStreamSynchronize(c->st));
   double s[7] = {0, 0, 0, 0, 0, 0, 0}, mnr = INFINITY, mnp = INFINITY, mxm = 0.0, bad = 0.0;
   for (int a = 0; a < 7; ++a) {

@@ -14,6 +14,8 @@ import pytest
 import workloads as W
 
 pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+SLOW = os.environ.get("STREAMS_SLOW", "0") == "1"        # opt-in full-size stepped configs 3 and 4 (minutes of oracle time)
 GAM = 1.4
 RHS_TOL = 1e-11
 STEP_TOL = 1e-9
@@ -28,7 +30,16 @@ def env():
     from paper_2004_02276_b200 import binding
     from oracle import binding as ob
     binding.lib()
-    return torch, binding, ob
+    yield torch, binding, ob
+    try:
+        import json
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        path = os.path.join(ROOT, "gpurun_out", "parity_numbers.json")
+        old = json.load(open(path)) if os.path.exists(path) else {}
+        old.update(RESULTS)
+        json.dump(old, open(path, "w"), indent=1)
+    except Exception:
+        pass
 
 
 def pair(env, wl):
@@ -41,24 +52,33 @@ def pair(env, wl):
     return o, g
 
 
-def rhs_scale(ro, w=None, lam=None):
-    """Per-variable scale of the RHS parity check (A18): max|R_oracle|, but never below
-    1e-3 * max|w_v| * lambda_max -- R_v is a sum of flux differences of size |w_v| lambda_max
-    (lambda_max = max (|u_d|+c)/h_d), and where those cancel to truncation level (the mass equation of a
-    solenoidal, uniform-density field: config 2) max|R_v| itself says nothing about round-off."""
-    sc = [np.abs(ro[v]).max() for v in range(5)]
-    if w is not None and lam is not None:
-        sc = [max(sc[v], 1e-3 * np.abs(w[v]).max() * lam) for v in range(5)]
-    return sc
+# (case, variable) pairs whose RHS error is measured against the cancellation floor of DESIGN.md A18 instead of
+# max|R_oracle,v|.  Everything else is STRICT (north_star: max|dR_v| / max|R_oracle,v| <= 1e-11).
+#   isotropic / mass: solenoidal velocity and uniform density, so R_rho = -div(rho u) is pure truncation error
+#   (max|R_rho| ~ 1e-5 of the flux differences it is the sum of) and says nothing about round-off: measured strict
+#   1.0e-9, against the floor 2.3e-13 (round 2, gpurun_out/parity_numbers.json -> DESIGN.md section 6).
+FLOOR_OK = {("isotropic", 0)}
+RESULTS = {}                                           # strict numbers of this session, dumped to gpurun_out/ at the end
 
 
-def rhs_err(rg, ro, w=None, lam=None):
-    sc = rhs_scale(ro, w, lam)
-    out = []
+def rhs_floor(w, lam):
+    """Cancellation floor of DESIGN.md A18: R_v is a sum of flux differences of size |w_v| lambda_max
+    (lambda_max = max (|u_d|+c)/h_d); 1e-3 of that."""
+    return [1e-3 * np.abs(w[v]).max() * lam for v in range(5)]
+
+
+def rhs_err(rg, ro, name, w=None, lam=None):
+    """Per variable: strict error max|dR_v| / max|R_oracle,v| and the error the test is held to (strict, except for
+    the allow-listed pairs, which use max(max|R_oracle,v|, floor))."""
+    strict, held = [], []
+    fl = rhs_floor(w, lam) if w is not None and lam is not None else [0.0] * 5
     for v in range(5):
         d = np.abs(rg[v] - ro[v]).max()
-        out.append(d / sc[v] if sc[v] > 0 else d)
-    return out
+        sc = np.abs(ro[v]).max()
+        strict.append(d / sc if sc > 0 else d)
+        sc_h = max(sc, fl[v]) if (name, v) in FLOOR_OK else sc
+        held.append(d / sc_h if sc_h > 0 else d)
+    return strict, held
 
 
 def l2_err(wg, wo):
@@ -75,8 +95,10 @@ def check_rhs(env, wl, tol=RHS_TOL):
     ro, rg = o.rhs(), g.rhs().cpu().numpy()
     assert np.isfinite(rg).all()
     lam = max(o.diagnostics(check=False).max_speed)
-    e = rhs_err(rg, ro, wl.state(), lam)
-    assert max(e) <= tol, (wl.name, e)
+    strict, held = rhs_err(rg, ro, wl.name, wl.state(), lam)
+    print("RHS %s %s: strict %s held %s" % (wl.name, list(wl.shape[1:]), ["%.2e" % e for e in strict], ["%.2e" % e for e in held]))
+    RESULTS["rhs:%s:%s" % (wl.name, "x".join(map(str, wl.shape[1:])))] = dict(strict=strict, held=held)
+    assert max(held) <= tol, (wl.name, strict, held)
     return o, g
 
 
@@ -100,6 +122,9 @@ def check_steps(env, wl, nsteps, tol=STEP_TOL):
     g.step(nsteps)
     wo, wg = o.get_state(), g.get_state().cpu().numpy()
     e = l2_err(wg, wo)
+    print("STEPS %s %s x%d: L2 %s" % (wl.name, list(wl.shape[1:]), nsteps, ["%.2e" % x for x in e]))
+    RESULTS["steps:%s:%s:%d" % (wl.name, "x".join(map(str, wl.shape[1:])), nsteps)] = dict(l2=e)
+    assert np.isfinite(wg).all()
     assert max(e) <= tol, (wl.name, e)
     do, dg = o.diagnostics(check=False), g.diagnostics(check=False)
     assert do.nonfinite == 0 and dg.nonfinite == 0
@@ -147,6 +172,8 @@ SMALL = {
     "channel_weno_forcing": lambda: mod(W.config3_channel(37, 19, 11), weno_enable=1, sensor_threshold=0.2, sensor_eps=0.1),
     # forcing with Dirichlet wall nodes (lazy forcing must leave the overridden wall rows alone)
     "channel_node_walls": lambda: mod(W.config3_channel(48, 24, 16), bc=NODE_WALLS),
+    # the paper's own channel numerics: 4th order, Sutherland, error-function grid
+    "channel_paper_small": lambda: W.config6_channel_paper(48, 24, 16),
 }
 
 STEPPED = ["channel_ragged", "channel_weno_forcing", "channel_node_walls", "sbli_weno_everywhere", "weno_mixed", "several_tiles_and_chunks"]
@@ -169,9 +196,11 @@ def test_steps_small(env, name):
     check_steps(env, SMALL[name](), 3)
 
 
-def test_uniform_flow_is_bitwise_steady(env):
-    """Free-stream preservation (oracle pin P3 is bitwise; the CUDA path shares z pair products between
-    nodes through running sums, so it is exact to round-off of the flux terms, not bitwise)."""
+def test_uniform_flow_is_steady_to_roundoff(env):
+    """Free-stream preservation.  The oracle's is bitwise (pin P3).  The CUDA path forms each node's flux difference
+    as phi_i sum(A_l - B_l) + sum(A_l phi_{i+l} - B_l phi_{i-l}) with fused multiply-adds; in uniform flow A_l = B_l
+    exactly but one product's rounding survives the two FMAs, so R is zero to round-off of the flux terms
+    (<= 1e-14 |w| lambda), not bitwise."""
     wl = W.random_periodic(40, 20, 12, amp=0.0, params=P())
     o, g = pair(env, wl)
     w0 = wl.state()
@@ -261,6 +290,56 @@ def test_split_stepping_is_bitwise_the_same(env):
         b.close()
 
 
+def test_statistics_gpu(env):
+    """SURVEY 8(f) rank 4 / PAPER.md:103: x-z plane means per wall-normal index, averaged over samples.  On the same
+    state the profiles agree with the oracle to summation round-off; sampled during a run (one sample per RK3 step)
+    to the accuracy of the states themselves."""
+    torch, binding, ob = env
+    for wl in (SMALL["channel_ragged"](), SMALL["sbli_small"](), W.config3_channel(256, 40, 72)):
+        o, g = pair(env, wl)
+        o.stats_accumulate()
+        g.stats_accumulate()
+        so, no = o.stats_read()
+        sg, ng = g.stats_read()
+        assert no == ng == 1
+        for m in range(16):
+            sc = max(np.abs(so[m]).max(), 1e-300)
+            assert np.abs(sg[m] - so[m]).max() <= 1e-13 * max(sc, np.abs(so[0]).max()), (wl.name, m)
+        for _ in range(3):
+            o.step(1)
+            g.step(1)
+            o.stats_accumulate()
+            g.stats_accumulate()
+        so, no = o.stats_read()
+        sg, ng = g.stats_read()
+        assert no == ng == 4
+        for m in range(16):
+            assert np.abs(sg[m] - so[m]).max() <= 1e-9 * max(np.abs(so[m]).max(), np.abs(so[0]).max()), (wl.name, m)
+        g.stats_reset()
+        assert g.stats_read()[1] == 0
+        g.close()
+        o.close()
+
+
+def test_graph_replay_equals_direct_launches(env):
+    """streams_step on a private stream replays one captured CUDA graph per step (grids below 2^24 nodes); on the
+    legacy default stream it launches kernel by kernel.  Same kernels, same order: bit-identical states."""
+    torch, binding, ob = env
+    for wl in (SMALL["channel_small"](), SMALL["weno_mixed"](), SMALL["channel_weno_forcing"](), SMALL["sbli_small"]()):
+        w0 = torch.from_numpy(wl.state()).cuda()
+        res = []
+        for stream in (None, torch.cuda.default_stream()):
+            g = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params, stream=stream)
+            g.set_state(w0)
+            g.step(1)
+            g.step(4)
+            torch.cuda.synchronize()
+            res.append((g.get_state().cpu().numpy(), g.diagnostics().dt, g.launch_count()))
+            g.close()
+        assert np.array_equal(res[0][0], res[1][0]), wl.name
+        assert res[0][1] == res[1][1] and res[0][2] == res[1][2]
+
+
 def test_sod_tube_gpu(env):
     """Hybrid recipe end to end on the GPU along x: same answer as the oracle after the full run."""
     n = 200
@@ -298,16 +377,26 @@ def test_config2_isotropic_full(env):
     print("config2: flagged interface fraction after 100 steps %.4f, initial flags %d" % (frac, nflag))
 
 
+def test_config6_channel_paper_literal(env):
+    """the channel with the paper's literal choices -- fourth-order flux and viscous terms
+    (PAPER.md:77, 83), Sutherland's law, error-function wall-normal mapping --
+    128x64x64: one RHS and 20 RK3 steps against the oracle."""
+    wl = W.config6_channel_paper()
+    check_rhs(env, wl)
+    o, g, do, dg = check_steps(env, wl, wl.steps)
+    assert abs(dg.forcing - do.forcing) <= 1e-9 * abs(do.forcing)
+
+
 def test_config3_channel(env):
     """config 3: channel with staggered walls and bulk forcing: reduced grid for the stated 200 steps,
-    and the full 256x128x128 grid for one RHS and 10 steps."""
+    and the full 256x128x128 grid for one RHS and 10 steps (the stated 200 at full size: test_config3_full_200_steps)."""
     wl = W.config3_channel(128, 64, 64)
     o, g, do, dg = check_steps(env, wl, wl.steps)
     assert abs(dg.forcing - do.forcing) <= 1e-9 * abs(do.forcing)
     full = W.config3_channel()
     check_rhs(env, full)
     o, g, do, dg = check_steps(env, full, 10)
-    d0 = None
+    assert abs(dg.forcing - do.forcing) <= 1e-9 * abs(do.forcing)
     # P11/P12 on the GPU path: mass and bulk momentum constant to round-off
     torch = env[0]
     g.set_state(torch.from_numpy(full.state()).cuda())
@@ -318,14 +407,34 @@ def test_config3_channel(env):
     assert abs(d1.mom[0] - d0.mom[0]) <= 1e-12 * abs(d0.mom[0])
 
 
-def slab_check(env, wl, gpu_rhs, slabs, planes=8):
+@pytest.mark.skipif(not SLOW, reason="opt-in (STREAMS_SLOW=1): about 5 minutes of oracle time")
+def test_config3_full_200_steps(env):
+    """config 3 at full size for the stated 200 RK3 steps (north_star: 1e-9 L2 after the stated step counts)."""
+    wl = W.config3_channel()
+    o, g, do, dg = check_steps(env, wl, wl.steps)
+    assert abs(dg.forcing - do.forcing) <= 1e-9 * abs(do.forcing)
+
+
+@pytest.mark.skipif(not SLOW, reason="opt-in (STREAMS_SLOW=1): about 20 minutes of oracle time and 12 GB of host memory")
+def test_config4_full_100_steps(env):
+    """config 4 at full size (1024x256x128) for the stated 100 RK3 steps with WENO active across the shock."""
+    wl = W.config4_sbli()
+    o, g, do, dg = check_steps(env, wl, wl.steps)
+    assert sum(dg.weno_ifaces) > 0
+    assert check_flags(env, o, g, sync=True) > 0
+
+
+def slab_check(env, wl, gpu_rhs, slabs, planes=8, gpu_minus=None):
     """Compare planes [k0, k0+planes) of a full-size GPU RHS with the oracle run on the slab plus `halo`
-    wrapped planes each side (forcing off on both sides).  Every stencil has z-radius 3; with the WENO
-    switch on, an interface flag looks at theta of nodes up to 3 planes away, each of which needs 3 more
-    planes, so the slab then carries 6."""
+    wrapped planes each side (forcing off in the oracle: a global reduction).  Every stencil has z-radius 3; with
+    the WENO switch on, an interface flag looks at theta of nodes up to 3 planes away, each of which needs 3 more
+    planes, so the slab then carries 6.  `gpu_minus(k0, k1)` (optional) returns what to subtract from the GPU planes
+    first (the body-force terms, when the GPU RHS was evaluated with forcing on).
+    Error per variable = max over the sampled planes of |dR_v| / max over the sampled planes of |R_oracle,v|:
+    the oracle's own scale (the full oracle field does not exist at this size), A18."""
     torch, binding, ob = env
-    worst = [0.0] * 5
-    scale = [float(gpu_rhs[v].abs().max()) for v in range(5)]
+    dmax = [0.0] * 5
+    scale = [0.0] * 5
     halo = 6 if wl.params["weno_enable"] else 3
     for k0 in slabs:
         sub = wl.slab(k0, k0 + planes, halo=halo)
@@ -333,9 +442,16 @@ def slab_check(env, wl, gpu_rhs, slabs, planes=8):
         o.set_state(sub.state())
         ro = o.rhs()[:, halo:halo + planes]
         rg = gpu_rhs[:, k0:k0 + planes].cpu().numpy()
+        assert np.isfinite(rg).all(), ("non-finite GPU residual in slab", k0)
+        if gpu_minus is not None:
+            rg = rg - gpu_minus(k0, k0 + planes)
         for v in range(5):
-            worst[v] = max(worst[v], np.abs(rg[v] - ro[v]).max() / scale[v])
+            dmax[v] = max(dmax[v], float(np.abs(rg[v] - ro[v]).max()))
+            scale[v] = max(scale[v], float(np.abs(ro[v]).max()))
         o.close()
+    worst = [dmax[v] / scale[v] for v in range(5)]
+    print("SLAB %s %s: strict %s" % (wl.name, slabs, ["%.2e" % e for e in worst]))
+    RESULTS["slab:%s:%s" % (wl.name, "x".join(map(str, wl.shape[1:])))] = dict(strict=worst)
     return worst
 
 
@@ -352,6 +468,7 @@ def test_config4_sbli(env):
     s = binding.Streams(full.grid, full.x, full.y, full.z, full.params)
     s.set_state(torch.from_numpy(full.state()).cuda())
     r = s.rhs()
+    assert bool(torch.isfinite(r).all())
     worst = slab_check(env, full, r, [0, 60, 120])
     assert max(worst) <= RHS_TOL, worst
     s.step(2)
@@ -360,28 +477,70 @@ def test_config4_sbli(env):
     s.close()
 
 
+def test_config5_geometry_stepped_with_forcing(env):
+    """The x-y launch geometry of config 5 (1024x512: 32 x 64 tiles, wall tiles, x-periodic edge tiles) with 64 planes,
+    which the oracle can step whole: two RK3 steps through the lazy-forcing path (k_rhs<2>, k_force_final,
+    k_force_fix, fused dt_next) against the oracle, forcing ON."""
+    wl = W.config3_channel(1024, 512, 64, seed=1005, name="channel_big_z64")
+    o, g, do, dg = check_steps(env, wl, 2)
+    assert abs(dg.forcing - do.forcing) <= 1e-9 * abs(do.forcing)
+
+
 def test_config5_big_channel_spot_check(env):
-    """config 5: 1024x512x512 (268M points) in the launch configuration bench.py times: one RHS checked
-    against the oracle on three 8-plane z-slabs; then invariants that hold at any size over 5 steps."""
+    """config 5: 1024x512x512 (268M points) in the launch configuration bench.py times, forcing ON:
+    * one RHS against the oracle on three 8-plane z-slabs, after removing f (e_rhou + u e_rhoE) with the GPU's f;
+    * the GPU's f against an independent extended-precision reduction of the GPU-produced R (S9), and the GPU's dt
+      against a NumPy maximum over the input state (S10) -- the two full-field reductions of SURVEY 8(d) row 5;
+    * then invariants that hold at any size over 5 steps."""
     torch, binding, ob = env
     wl = W.config5_channel_big()
     if torch.cuda.get_device_properties(0).total_memory < 70e9:
         pytest.skip("needs ~55 GB of device memory")
-    nofo = dict(wl.params, forcing=0)
-    s = binding.Streams(wl.grid, wl.x, wl.y, wl.z, nofo)
+    nx, ny, nz = wl.grid["nx"], wl.grid["ny"], wl.grid["nz"]
+    # metrics exactly as S2 defines them (index derivative of the coordinates), from the oracle on a thin grid
+    thin = wl.slab(0, 1, halo=0)
+    om = ob.Oracle(thin.grid, thin.x, thin.y, thin.z, thin.params)
+    hx, hy = om.metrics(0)[0], om.metrics(1)[0]
+    hz = wl.grid["len"][2] / nz
+    om.close()
+    s = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
     w = torch.empty(wl.shape, dtype=torch.float64, device="cuda")
-    for k0 in range(0, wl.grid["nz"], 16):
-        w[:, k0:k0 + 16].copy_(torch.from_numpy(wl.state(k0, k0 + 16)))
+    lam_max = 0.0                                       # S10 from the input state, NumPy, slab by slab
+    for k0 in range(0, nz, 16):
+        ws = wl.state(k0, k0 + 16)
+        w[:, k0:k0 + 16].copy_(torch.from_numpy(ws))
+        rho = ws[0]
+        vel = [ws[1] / rho, ws[2] / rho, ws[3] / rho]
+        pr = (GAM - 1.0) * (ws[4] - 0.5 * rho * (vel[0] ** 2 + vel[1] ** 2 + vel[2] ** 2))
+        c = np.sqrt(GAM * pr / rho)
+        lam_max = max(lam_max, float(((np.abs(vel[0]) + c) / hx[None, None, :]).max()),
+                      float(((np.abs(vel[1]) + c) / hy[None, :, None]).max()), float(((np.abs(vel[2]) + c) / hz).max()))
     s.set_state(w)
     r = s.rhs()
-    worst = slab_check(env, wl, r, [0, 252, 504])
+    f = s.diagnostics().forcing
+    assert f > 0.0
+
+    def force_terms(k0, k1):
+        u = (w[1, k0:k1] / w[0, k0:k1]).cpu().numpy()
+        out = np.zeros((5,) + u.shape)
+        out[1] = f
+        out[4] = f * u
+        return out
+
+    worst = slab_check(env, wl, r, [0, 252, 504], gpu_minus=force_terms)
     assert max(worst) <= RHS_TOL, worst
-    # full-field forcing sum against an independent float64 pairwise/fsum reduction of the GPU-produced R
-    hx = np.full(wl.grid["nx"], wl.grid["len"][0] / wl.grid["nx"])
-    s.close()
+    # S9: f = -sum(R0_rhou vol) / sum(vol) with R0 = R - f, summed in extended precision plane by plane
+    volxy = torch.from_numpy(hy[:, None] * hx[None, :]).cuda()
+    num, den = [], []
+    for k in range(nz):
+        plane = ((r[1, k] - f) * volxy).cpu().numpy()
+        num.append(float(np.sum(plane, dtype=np.longdouble)) * hz)
+        den.append(float(np.sum(hy[:, None] * hx[None, :], dtype=np.longdouble)) * hz)
+    f_ref = -math.fsum(num) / math.fsum(den)
+    print("config5: f gpu %.15e  reference %.15e" % (f, f_ref))
+    RESULTS["config5:forcing"] = dict(gpu=f, reference=f_ref)
+    assert abs(f - f_ref) <= 1e-11 * abs(f_ref)
     del r
-    s = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
-    s.set_state(w)
     d0 = s.diagnostics()
     s.step(5)
     d1 = s.diagnostics()
@@ -389,5 +548,11 @@ def test_config5_big_channel_spot_check(env):
     assert abs(d1.mass - d0.mass) <= 1e-13 * d0.mass
     assert abs(d1.mom[0] - d0.mom[0]) <= 1e-12 * abs(d0.mom[0])
     assert abs(d0.volume - 6 * math.pi * 2 * 2 * math.pi) < 1e-6 * d0.volume
-    assert hx[0] > 0
+    # S10: the first step's dt against the NumPy maximum (dt of later steps is carried on the device)
+    s.set_state(w)
+    s.step(1)
+    dt = s.diagnostics().dt
+    print("config5: dt gpu %.15e  reference %.15e" % (dt, wl.params["cfl"] / lam_max))
+    RESULTS["config5:dt"] = dict(gpu=dt, reference=wl.params["cfl"] / lam_max)
+    assert abs(dt - wl.params["cfl"] / lam_max) <= 1e-13 * dt
     s.close()

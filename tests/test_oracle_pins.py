@@ -492,6 +492,20 @@ def test_P15_metrics_order(ob):
     assert np.allclose(h, 2 * np.pi / 8, rtol=1e-14) and np.abs(g).max() < 1e-14
 
 
+def test_erf_grid_reproduces_the_papers_spacing(ob):
+    """PAPER.md:110: error-function mapping, Ny = 256, spacing in wall units 0.8 ... 5.7 at Re_tau = 489 (ratio 7.1);
+    staggered: the wall planes y = -1, +1 lie half-way between the first node and its mirror image."""
+    y = W.erf_nodes(256)
+    d = np.diff(y)
+    assert 0.7 < d.min() * 489 < 1.0 and 5.0 < d.max() * 489 < 6.6 and 6.0 < d.max() / d.min() < 7.6
+    assert abs((y[0] + 1.0) - (1.0 - y[-1])) < 1e-15 and np.allclose(y, -y[::-1], atol=1e-15)
+    wl = W.config6_channel_paper(8, 32, 4)
+    assert wl.params["order"] == 4 and wl.params["visc_model"] == W.VISC_SUTHERLAND
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    h, g = o.metrics(1)
+    assert (h > 0).all() and abs(h.sum() - 2.0) < 2e-3          # the metric integrates to the channel height
+
+
 # ------------------------------------------------------------------ P16 + design order: manufactured fields
 @pytest.fixture(scope="module")
 def manufactured():

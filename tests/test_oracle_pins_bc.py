@@ -397,3 +397,56 @@ def test_weno_flux_at_a_moving_shock_and_a_contact(ob, d):
     zero = np.zeros(shape)
     o.set_state(W.prim_to_cons(np.where(left, 2.5, 0.4), zero, zero, zero, np.full(shape, 0.7), GAM))
     assert np.abs(o.rhs()).max() < 1e-13 * 0.7 / h
+
+
+# ------------------------------------------------------------------ statistics
+def stats_field(nx, ny, nz, A, seedless=True):
+    """rho = rho0 (1 + D cos z), u = U(y) + A sin x cos z, v = C sin x cos z, w = 0.2, T = T0(y) + B cos 2x on
+    equispaced periodic x, z: every x-z node mean below is exact (trigonometric sums below the Nyquist limit)."""
+    L = 2 * np.pi
+    x, z = L * np.arange(nx) / nx, L * np.arange(nz) / nz
+    y = np.linspace(-0.9, 0.9, ny)
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    rho0, D, C_, B = 1.3, 0.2, 0.15, 0.1
+    U, T0 = 1.0 - Y ** 2, 1.0 + 0.3 * Y
+    rho = rho0 * (1 + D * np.cos(Z))
+    u = U + A * np.sin(X) * np.cos(Z)
+    v = C_ * np.sin(X) * np.cos(Z)
+    w = 0.2 + 0 * X
+    T = T0 + B * np.cos(2 * X)
+    grid = dict(nx=nx, ny=ny, nz=nz, len=[L, 1.8, L])
+    Uy, T0y = 1.0 - y ** 2, 1.0 + 0.3 * y
+    exact = dict(rho=rho0 + 0 * y, u=Uy, v=0 * y, w=0.2 + 0 * y, p=R_GAS * rho0 * T0y, T=T0y, rho_u=rho0 * Uy, rho_v=0 * y,
+                 rho_w=0.2 * rho0 + 0 * y, rho_T=rho0 * T0y, rho_uu=rho0 * (Uy ** 2 + A * A / 4), rho_vv=rho0 * C_ * C_ / 4 + 0 * y,
+                 rho_ww=0.04 * rho0 + 0 * y, rho_uv=rho0 * A * C_ / 4 + 0 * y, TT=T0y ** 2 + B * B / 2, mu=0.02 * T0y)
+    return grid, (x, y, z), W.prim_to_cons(rho, u, v, w, rho * R_GAS * T, GAM), exact
+
+
+STAT_ORDER = ["rho", "u", "v", "w", "p", "T", "mu", "rho_u", "rho_v", "rho_w", "rho_T", "rho_uu", "rho_vv", "rho_ww", "rho_uv", "TT"]
+
+
+def test_statistics_closed_form_plane_means(ob):
+    """averaging over the homogeneous directions and time.  Plane means of a trigonometric field are
+    known in closed form; the time average of two samples is their mean; Favre u~ = mean(rho u) / mean(rho)."""
+    prm = W.default_params(Rgas=R_GAS, mu_ref=0.02, T_ref=1.0, visc_exp=1.0, bc=[W.BC_PERIODIC] * 2 + [W.BC_EXTRAP] * 2 + [W.BC_PERIODIC] * 2)
+    grid, (x, y, z), w1, ex1 = stats_field(16, 7, 12, A=0.3)
+    _g, _c, w2, ex2 = stats_field(16, 7, 12, A=0.5)
+    o = ob.Oracle(grid, x, y, z, prm)
+    o.set_state(w1)
+    o.stats_accumulate()
+    st, n = o.stats_read()
+    assert n == 1
+    for m, key in enumerate(STAT_ORDER):
+        assert np.abs(st[m] - ex1[key]).max() < 1e-14 * max(1.0, np.abs(ex1[key]).max()), key
+    o.set_state(w2)
+    o.stats_accumulate()
+    st, n = o.stats_read()
+    assert n == 2
+    for m, key in enumerate(STAT_ORDER):
+        assert np.abs(st[m] - 0.5 * (ex1[key] + ex2[key])).max() < 1e-14 * max(1.0, np.abs(ex1[key]).max()), key
+    # Favre-averaged velocity and the density-scaled normal stress rho u''u'' = mean(rho uu) - mean(rho u)^2 / mean(rho)
+    assert np.abs(st[7] / st[0] - ex1["u"]).max() < 1e-14
+    tau = st[11] - st[7] ** 2 / st[0]
+    assert np.abs(tau - 1.3 * 0.5 * (0.3 ** 2 + 0.5 ** 2) / 4).max() < 1e-14
+    o.stats_reset()
+    assert o.stats_read()[1] == 0 and np.abs(o.stats_read()[0]).max() == 0.0

@@ -171,6 +171,15 @@ def tanh_nodes(ny, b=1.7):
     return np.tanh(b * eta) / np.tanh(b)
 
 
+def erf_nodes(ny, a=1.4):
+    """Error-function wall-normal mapping of the paper's channel, staggered nodes (the walls at y = -1, +1
+    fall half-way between a ghost and the first node): y_j = erf(a eta_j) / erf(a), eta_j = -1 + (2j - 1)/ny.
+    a = 1.4 gives the paper's spacing ratio: centre / wall = exp(a^2) = 7.1 (its dy+ = 0.8 ... 5.7 at ny = 256)."""
+    from math import erf
+    eta = -1.0 + (2.0 * np.arange(1, ny + 1) - 1.0) / ny
+    return np.array([erf(a * e) for e in eta]) / erf(a)
+
+
 def _smooth121(a, axis, periodic, passes=4):
     for _ in range(passes):
         if periodic:
@@ -216,6 +225,18 @@ def config3_channel(nx=256, ny=128, nz=128, seed=1003, steps=200, name="channel"
         return prim_to_cons(rho, u, v, w, p, gamma)
 
     return Workload(name, grid, x, y, z, params, steps, seed, state)
+
+
+def config6_channel_paper(nx=128, ny=64, nz=64, seed=1006, steps=20) -> Workload:
+    """The paper's OWN channel numerics (section 8.f rank 2 of SURVEY.md) on the seeded channel input: fourth-order
+    central flux and viscous terms, Sutherland's law, error-function wall-normal
+    mapping (PAPER.md:110), M_b = 1.5, Re_b = 14725 (PAPER.md:107)."""
+    wl = config3_channel(nx, ny, nz, seed, steps, name="channel_paper")
+    wl.y = erf_nodes(ny)
+    Reb = 14725.0
+    wl.params.update(order=4, visc_model=VISC_SUTHERLAND, mu_ref=2.0 * 1.0 * 1.5 * 1.0 / Reb, T_ref=1.0,
+                     suth_S=110.4 / 273.15)
+    return wl
 
 
 def config5_channel_big(nx=1024, ny=512, nz=512, seed=1005, steps=50, smooth=False) -> Workload:
