@@ -300,7 +300,7 @@ def run_ours(args, rank, world, local_rank):
                "config": {"workload": wl.name, "grid": [wl.grid["nx"], wl.grid["ny"], wl.grid["nz"]], "points": npts,
                           "order": wl.params["order"], "forcing": wl.params["forcing"], "weno": wl.params["weno_enable"],
                           "parallelism": "replicas only" if world > 1 else "1 GPU",
-                          "l2": "state (10.7 GB) and RK register larger than the 126 MB L2; no flush needed"
+                          "l2": "state (%.2f GB) and RK register larger than the 126 MB L2; no flush needed" % (state_bytes / 1e9)
                           if state_bytes > 2 * 126e6 else "inputs smaller than L2 (launch-latency regime)"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                "roofline": {"bound": "alu" if t_alu >= t_hbm else "hbm", "kernel": "k_rhs", "achieved": alu_achieved, "peak": alu_peak,

@@ -58,10 +58,14 @@ enum {
   STREAMS_BC_WALL_ISO_NODE = 2,      /* isothermal no-slip wall on the boundary node */
   STREAMS_BC_INFLOW_FROZEN = 3,      /* Dirichlet ghost planes frozen at set_state (stands in for the
                                         digital-filter inflow of PAPER.md:126, A16) */
-  STREAMS_BC_OUTFLOW_NR = 4,         /* characteristic non-reflecting boundary   */
+  STREAMS_BC_OUTFLOW_NR = 4,         /* characteristic non-reflecting boundary: xmax (outflow) or ymax (upper boundary) */
   STREAMS_BC_SHOCKGEN = 5,           /* inviscid oblique-shock state imposed in the ghosts of ymax
                                                                                  */
-  STREAMS_BC_EXTRAP = 6              /* zeroth-order extrapolation (1-D tube tests)            */
+  STREAMS_BC_EXTRAP = 6,             /* zeroth-order extrapolation (1-D tube tests)            */
+  STREAMS_BC_WALL_ISO_CHAR = 7       /* ymin only: isothermal no-slip wall on the boundary node with the "similar
+                                        characteristic wave treatment" of PAPER.md:126: the wall-normal convective
+                                        derivative at the wall node in characteristic form, incoming acoustic wave =
+                                        reflection of the outgoing one (A14b)        */
 };
 
 enum { STREAMS_VISC_POWER = 0, STREAMS_VISC_SUTHERLAND = 1 };

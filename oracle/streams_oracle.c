@@ -189,10 +189,11 @@ static int check_params(const oracle_grid* g, const oracle_params* p) {
     if (lo == ORC_BC_PERIODIC && !(g->len[d] > 0.0)) return 0;
     for (int s = 0; s < 2; ++s) {
       int b = p->bc[2 * d + s];
-      if (b < 0 || b > ORC_BC_EXTRAP) return 0;
+      if (b < 0 || b > ORC_BC_WALL_CHAR) return 0;
       if ((b == ORC_BC_WALL_STAG || b == ORC_BC_WALL_NODE) && d != 1) return 0;
+      if (b == ORC_BC_WALL_CHAR && !(d == 1 && s == 0)) return 0;
       if (b == ORC_BC_INFLOW && !(d == 0 && s == 0)) return 0;
-      if (b == ORC_BC_OUTFLOW && !(d == 0 && s == 1)) return 0;
+      if (b == ORC_BC_OUTFLOW && !((d == 0 || d == 1) && s == 1)) return 0;
       if (b == ORC_BC_SHOCKGEN && !(d == 1 && s == 1)) return 0;
     }
   }
@@ -335,7 +336,8 @@ static void fill_ghosts(oracle_ctx* c) {
             switch (bc) {
               case ORC_BC_PERIODIC: src = imod(gi, n); break;
               case ORC_BC_WALL_STAG: src = s == 0 ? l - 1 : n - l; break;
-              case ORC_BC_WALL_NODE: src = s == 0 ? l : n - 1 - l; break;
+              case ORC_BC_WALL_NODE:
+              case ORC_BC_WALL_CHAR: src = s == 0 ? l : n - 1 - l; break;
               default: src = s == 0 ? 0 : n - 1; break;
             }
             id[d] = src;
@@ -343,7 +345,8 @@ static void fill_ghosts(oracle_ctx* c) {
             for (int v = 0; v < NV; ++v) ws[v] = c->wg[v * NP + so];
             switch (bc) {
               case ORC_BC_WALL_STAG:
-              case ORC_BC_WALL_NODE: reflect_wall(p, p->T_wall[s], ws, wo); break;
+              case ORC_BC_WALL_NODE:
+              case ORC_BC_WALL_CHAR: reflect_wall(p, p->T_wall[s], ws, wo); break;
               case ORC_BC_INFLOW:
                 /* d == 0, s == 0: transverse indices are interior here because x is filled first */
                 for (int v = 0; v < NV; ++v) wo[v] = c->inflow[((size_t)v * c->n[2] + id[2]) * c->n[1] + id[1]];
@@ -583,6 +586,7 @@ static void convective(oracle_ctx* c, double* R) {
     const int per = is_periodic(c, d);
     const int stag_lo = c->p.bc[2 * d] == ORC_BC_WALL_STAG, stag_hi = c->p.bc[2 * d + 1] == ORC_BC_WALL_STAG;
     const int outflow_hi = c->p.bc[2 * d + 1] == ORC_BC_OUTFLOW;
+    const int charwall_lo = c->p.bc[2 * d] == ORC_BC_WALL_CHAR;
     long long nflag = 0;
 #pragma omp parallel for reduction(+ : nflag)
     for (int t2 = 0; t2 < c->n[e2]; ++t2) {
@@ -616,6 +620,31 @@ static void convective(oracle_ctx* c, double* R) {
               for (int v = 0; v < 5; ++v) acc += Lm[sc * 5 + v] * dw[v];
               Ls[sc] = lam[sc] >= 0.0 ? lam[sc] * acc : 0.0;
             }
+            for (int v = 0; v < NV; ++v) {
+              double acc = 0.0;
+              for (int sc = 0; sc < 5; ++sc) acc += Rm[v * 5 + sc] * Ls[sc];
+              R[v * np + oi] -= acc;
+            }
+          } else if (charwall_lo && i == 0) {
+            /* Characteristic wave treatment at the no-slip wall (reading A14b): one-sided dw into the
+               domain, the wave leaving through the wall (lambda_1 = u_n - c <= 0) is computed from the interior, the
+               incoming acoustic wave is its reflection L_5 = L_1 (no normal momentum is created: with u_n = 0,
+               -(r_1 L_1 + r_5 L_5) has no wall-normal momentum component), entropy and shear waves do not enter
+               (lambda = u_n = 0 at the wall; removed if positive). */
+            const size_t ob = GI(c, id[0], id[1], id[2]);
+            const size_t s = c->sd[d];
+            double dw[5], Lm[25], Rm[25], lam[5], ub[3];
+            for (int v = 0; v < NV; ++v)
+              dw[v] = (-3.0 * c->wg[v * NP + ob] + 4.0 * c->wg[v * NP + ob + s] - c->wg[v * NP + ob + 2 * s]) / (2.0 * c->h[d][i]);
+            for (int m = 0; m < 3; ++m) ub[m] = c->q[(Q_U + m) * NP + ob];
+            oracle_eigen(d, c->p.gamma, ub, c->q[Q_H * NP + ob], Lm, Rm, lam);
+            double Ls[5];
+            for (int sc = 0; sc < 5; ++sc) {
+              double acc = 0.0;
+              for (int v = 0; v < 5; ++v) acc += Lm[sc * 5 + v] * dw[v];
+              Ls[sc] = lam[sc] <= 0.0 ? lam[sc] * acc : 0.0;
+            }
+            Ls[4] = Ls[0];
             for (int v = 0; v < NV; ++v) {
               double acc = 0.0;
               for (int sc = 0; sc < 5; ++sc) acc += Rm[v * 5 + sc] * Ls[sc];
@@ -843,7 +872,7 @@ int oracle_step(oracle_ctx* c, int nsteps) {
       double* t = c->Rprev; c->Rprev = c->Rcur; c->Rcur = t;
       /* S1 node wall: after every stage rho u = rho v = rho w = 0, rho E = rho cv Tw (rho evolves by the scheme) */
       for (int s = 0; s < 2; ++s)
-        if (c->p.bc[2 + s] == ORC_BC_WALL_NODE) {
+        if (c->p.bc[2 + s] == ORC_BC_WALL_NODE || c->p.bc[2 + s] == ORC_BC_WALL_CHAR) {
           const int j = s == 0 ? 0 : c->n[1] - 1;
           for (int k = 0; k < c->n[2]; ++k)
             for (int i = 0; i < c->n[0]; ++i) {

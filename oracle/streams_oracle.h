@@ -19,7 +19,7 @@ extern "C" {
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENONFINITE = -4, ORC_ESTATE = -5 };
 enum { ORC_BC_PERIODIC = 0, ORC_BC_WALL_STAG = 1, ORC_BC_WALL_NODE = 2, ORC_BC_INFLOW = 3,
-       ORC_BC_OUTFLOW = 4, ORC_BC_SHOCKGEN = 5, ORC_BC_EXTRAP = 6 };
+       ORC_BC_OUTFLOW = 4, ORC_BC_SHOCKGEN = 5, ORC_BC_EXTRAP = 6, ORC_BC_WALL_CHAR = 7 };
 enum { ORC_VISC_POWER = 0, ORC_VISC_SUTHERLAND = 1 };
 enum { ORC_NSTAT = 16 };   /* statistics per wall-normal index, see oracle_stats_accumulate */
 

@@ -18,7 +18,7 @@ namespace streams {
 constexpr int HALO = 3;
 constexpr int NQ = 7;                 // stored primitives per node
 
-enum { BC_PERIODIC = 0, BC_WALL_STAG = 1, BC_WALL_NODE = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_SHOCKGEN = 5, BC_EXTRAP = 6 };
+enum { BC_PERIODIC = 0, BC_WALL_STAG = 1, BC_WALL_NODE = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_SHOCKGEN = 5, BC_EXTRAP = 6, BC_WALL_CHAR = 7 };
 enum { VISC_POWER = 0, VISC_SUTH = 1 };
 
 // central coefficients of order 2L, zero-padded to three entries
@@ -107,6 +107,9 @@ __device__ __forceinline__ void wall_node_override(const DevP& P, double Tw, dou
   q.u = 0.0; q.v = 0.0; q.w = 0.0; q.T = Tw; q.mu = mu_w; q.H = P.cp * Tw;
 }
 
+// wall on the boundary node (Dirichlet override after every stage): plain reflected-ghost wall or its characteristic variant
+__device__ __forceinline__ bool node_wall(int bc) { return bc == BC_WALL_NODE || bc == BC_WALL_CHAR; }
+
 // index maps ----------------------------------------------------------------------------------
 // x: returns source index; inflow=true means "take the frozen inflow plane"
 __device__ __forceinline__ int map_x(const DevP& P, int i, bool& inflow) {
@@ -130,7 +133,7 @@ __device__ __forceinline__ int map_y(const DevP& P, int j, int& mode) {
     const int b = P.bc[2];
     if (b == BC_PERIODIC) return wrap(j, P.ny);
     if (b == BC_WALL_STAG) { mode = 1; return -j - 1; }
-    if (b == BC_WALL_NODE) { mode = 1; return -j; }
+    if (b == BC_WALL_NODE || b == BC_WALL_CHAR) { mode = 1; return -j; }
     return 0;
   }
   if (j >= P.ny) {

@@ -75,8 +75,8 @@ __global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, d
     advance_prim(P, q, dW);
     int i_, j, k_;
     node_ijk(P, o, i_, j, k_);
-    if (j == 0 && P.bc[2] == BC_WALL_NODE) wall_node_override(P, P.Twall[0], P.mu_wall[0], q);
-    if (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE) wall_node_override(P, P.Twall[1], P.mu_wall[1], q);
+    if (j == 0 && node_wall(P.bc[2])) wall_node_override(P, P.Twall[0], P.mu_wall[0], q);
+    if (j == P.ny - 1 && node_wall(P.bc[3])) wall_node_override(P, P.Twall[1], P.mu_wall[1], q);
     Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu; Q[o + 6 * P.N] = q.H;
   }
 }
@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(RT) k_force_fix(const __grid_constant__ DevP P
                                                   const DevScal* __restrict__ sc, double beta, double* __restrict__ speed) {
   __shared__ double sh[RT / 32];
   const double c = sc->dt * beta * sc->force;
-  const bool wn0 = P.bc[2] == BC_WALL_NODE, wn1 = P.bc[3] == BC_WALL_NODE;
+  const bool wn0 = node_wall(P.bc[2]), wn1 = node_wall(P.bc[3]);
   const int nrows = P.ny * P.nz;
   double m[3] = {0.0, 0.0, 0.0};
   for (int row = blockIdx.x; row < nrows; row += gridDim.x) {

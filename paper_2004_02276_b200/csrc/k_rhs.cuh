@@ -298,40 +298,50 @@ __device__ __forceinline__ void visc_assemble(const DevP& P, const Nb& c, NodeAc
   N.R[4] += fma(c.u, V0, fma(c.v, V1, c.w * V2)) + Phi + heat;
 }
 
-// S8: characteristic form of the x-derivative at the outflow node, incoming waves removed.
-// Replaces the index-space flux difference f of the x direction.  Rare path (one column): kept out of line.
+// S8: characteristic form of the derivative along D at a boundary node, incoming waves removed.
+// Replaces the index-space flux difference f of direction D.  side = +1: max-index face (one-sided difference
+// backwards, waves with lambda >= 0 leave), side = -1: min-index face (forwards, lambda <= 0 leave).  wall = true:
+// characteristic wall (reading A14b): the incoming acoustic wave is the reflection of the outgoing one, L_5 = L_1.
+// Rare path (one column / row): kept out of line.
 struct F5 { double v[5]; };   // returned by value: stays in registers across the call (no local-memory frame)
-__device__ __noinline__ F5 outflow_x(const DevP& P, const double* __restrict__ t, int oc) {
+template <int D>
+__device__ __noinline__ F5 char_face(const DevP& P, const double* __restrict__ t, int oc, int st, int side, bool wall) {
   F5 r;
   double* f = r.v;
-  const Nb c = tile_nb(t, oc), n1 = tile_nb(t, oc - 1), n2 = tile_nb(t, oc - 2);
+  const Nb c = tile_nb(t, oc), n1 = tile_nb(t, oc - side * st), n2 = tile_nb(t, oc - 2 * side * st);
   const double pc = c.rho * (P.Rgas * c.T), p1 = n1.rho * (P.Rgas * n1.T), p2 = n2.rho * (P.Rgas * n2.T);
   const double w0[5] = {c.rho, c.rho * c.u, c.rho * c.v, c.rho * c.w, c.rho * c.H - pc};
   const double w1[5] = {n1.rho, n1.rho * n1.u, n1.rho * n1.v, n1.rho * n1.w, n1.rho * n1.H - p1};
   const double w2[5] = {n2.rho, n2.rho * n2.u, n2.rho * n2.v, n2.rho * n2.w, n2.rho * n2.H - p2};
   double dw[5];
+  const double sg = (double)side;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) dw[v] = (3.0 * w0[v] - 4.0 * w1[v] + w2[v]) * 0.5;   // * ihx by the caller
-  const double u = c.u, v_ = c.v, w_ = c.w;
-  const double q2 = u * u + v_ * v_ + w_ * w_;
+  for (int v = 0; v < 5; ++v) dw[v] = sg * (3.0 * w0[v] - 4.0 * w1[v] + w2[v]) * 0.5;   // * ih by the caller
+  constexpr int T1 = (D + 1) % 3, T2 = (D + 2) % 3;
+  const double vel[3] = {c.u, c.v, c.w};
+  const double un = vel[D];
+  const double q2 = c.u * c.u + c.v * c.v + c.w * c.w;
   const double Hc = P.cp * c.T + 0.5 * q2;
   const double c2 = P.gm1 * (Hc - 0.5 * q2), cs = sqrt(c2);
   const double bb1 = P.gm1 / c2, bb2 = 0.5 * q2 * bb1;
-  const double mdw = u * dw[1] + v_ * dw[2] + w_ * dw[3];
+  const double mdw = c.u * dw[1] + c.v * dw[2] + c.w * dw[3];
   double Ls[5];
-  Ls[0] = 0.5 * ((bb2 + u / cs) * dw[0] - bb1 * mdw - dw[1] / cs + bb1 * dw[4]);
+  Ls[0] = 0.5 * ((bb2 + un / cs) * dw[0] - bb1 * mdw - dw[1 + D] / cs + bb1 * dw[4]);
   Ls[1] = (1.0 - bb2) * dw[0] + bb1 * mdw - bb1 * dw[4];
-  Ls[2] = -v_ * dw[0] + dw[2];
-  Ls[3] = -w_ * dw[0] + dw[3];
-  Ls[4] = 0.5 * ((bb2 - u / cs) * dw[0] - bb1 * mdw + dw[1] / cs + bb1 * dw[4]);
-  const double lam[5] = {u - cs, u, u, u, u + cs};
+  Ls[2] = -vel[T1] * dw[0] + dw[1 + T1];
+  Ls[3] = -vel[T2] * dw[0] + dw[1 + T2];
+  Ls[4] = 0.5 * ((bb2 - un / cs) * dw[0] - bb1 * mdw + dw[1 + D] / cs + bb1 * dw[4]);
+  const double lam[5] = {un - cs, un, un, un, un + cs};
 #pragma unroll
-  for (int m = 0; m < 5; ++m) Ls[m] = lam[m] >= 0.0 ? lam[m] * Ls[m] : 0.0;
-  f[0] = Ls[0] + Ls[1] + Ls[4];
-  f[1] = (u - cs) * Ls[0] + u * Ls[1] + (u + cs) * Ls[4];
-  f[2] = v_ * Ls[0] + v_ * Ls[1] + Ls[2] + v_ * Ls[4];
-  f[3] = w_ * Ls[0] + w_ * Ls[1] + Ls[3] + w_ * Ls[4];
-  f[4] = (Hc - u * cs) * Ls[0] + 0.5 * q2 * Ls[1] + v_ * Ls[2] + w_ * Ls[3] + (Hc + u * cs) * Ls[4];
+  for (int m = 0; m < 5; ++m) Ls[m] = (side > 0 ? lam[m] >= 0.0 : lam[m] <= 0.0) ? lam[m] * Ls[m] : 0.0;
+  if (wall) Ls[4] = Ls[0];
+  const double sm = Ls[0] + Ls[1] + Ls[4];
+  f[0] = sm;
+  f[1] = c.u * sm; f[2] = c.v * sm; f[3] = c.w * sm;
+  f[1 + D] += cs * (Ls[4] - Ls[0]);
+  f[1 + T1] += Ls[2];
+  f[1 + T2] += Ls[3];
+  f[4] = (Hc - un * cs) * Ls[0] + 0.5 * q2 * Ls[1] + vel[T1] * Ls[2] + vel[T2] * Ls[3] + (Hc + un * cs) * Ls[4];
   return r;
 }
 
@@ -578,7 +588,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
           double f[5];
           conv_from_acc<0>(c, X, f);
           if (!PLAIN && gi == P.nx - 1 && P.bc[1] == BC_OUTFLOW) {
-            const F5 r = outflow_x(*sP, t, loc);
+            const F5 r = char_face<0>(*sP, t, loc, 1, 1, false);
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
           }
@@ -600,6 +610,12 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
           const bool wall_hi = gj == P.ny - 1 && P.bc[3] == BC_WALL_STAG;
           if (!PLAIN && (wall_lo || wall_hi)) {
             const F5 r = wall_y(*sP, t, loc, wall_lo, wall_hi);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) f[v] = r.v[v];
+          }
+          const bool nr_top = gj == P.ny - 1 && P.bc[3] == BC_OUTFLOW, ch_wall = gj == 0 && P.bc[2] == BC_WALL_CHAR;
+          if (!PLAIN && (nr_top || ch_wall)) {
+            const F5 r = char_face<1>(*sP, t, loc, PITCH, nr_top ? 1 : -1, ch_wall);
 #pragma unroll
             for (int v = 0; v < 5; ++v) f[v] = r.v[v];
           }
@@ -684,8 +700,8 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         Prim qn; qn.rho = rw[0]; qn.u = uw[0]; qn.v = vw[0]; qn.w = ww[0]; qn.T = Tw[0]; qn.mu = mw[0]; qn.H = 0.0;
         bool store_mu = !LAZY;
         advance_prim<!LAZY>(P, qn, dW);
-        if (!PLAIN && gj == 0 && P.bc[2] == BC_WALL_NODE) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
-        if (!PLAIN && gj == P.ny - 1 && P.bc[3] == BC_WALL_NODE) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
+        if (!PLAIN && gj == 0 && node_wall(P.bc[2])) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
+        if (!PLAIN && gj == P.ny - 1 && node_wall(P.bc[3])) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
         A.q_out[o] = qn.rho; A.q_out[o + P.N] = qn.u; A.q_out[o + 2 * P.N] = qn.v; A.q_out[o + 3 * P.N] = qn.w;
         A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 6 * P.N] = qn.H;
         if (store_mu) A.q_out[o + 5 * P.N] = qn.mu;
@@ -750,8 +766,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const int i0 = cta.x * TX, j0 = cta.y * TY;
   const bool inside = i0 + TX <= P.nx && j0 + TY <= P.ny;
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
-  const bool wall_lo = (P.bc[2] == BC_WALL_STAG || P.bc[2] == BC_WALL_NODE) && j0 == 0;
-  const bool wall_hi = (P.bc[3] == BC_WALL_STAG || P.bc[3] == BC_WALL_NODE) && j0 + TY >= P.ny;
+  const bool wall_lo = (P.bc[2] == BC_WALL_STAG || node_wall(P.bc[2])) && j0 == 0;
+  const bool wall_hi = (P.bc[3] == BC_WALL_STAG || node_wall(P.bc[3]) || P.bc[3] == BC_OUTFLOW) && j0 + TY >= P.ny;
   if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, tmap, sm, cta);
   else rhs_body<MODE, false>(P, A, tmap, sm, cta);
 }

@@ -51,23 +51,6 @@ __global__ void __launch_bounds__(RT) k_sensor(const __grid_constant__ DevP P, c
   if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned long long*>(&sc->max_theta), (unsigned long long)__double_as_longlong(t));
 }
 
-// node flag at a (possibly ghost) index along direction d: periodic wrap, else nearest interior node (A17)
-__device__ __forceinline__ int nflag_at(const DevP& P, const unsigned char* __restrict__ nflag, int d, int i, int j, int k, int g) {
-  const int n = d == 0 ? P.nx : (d == 1 ? P.ny : P.nz);
-  const int gg = P.bc[2 * d] == BC_PERIODIC ? wrap(g, n) : min(max(g, 0), n - 1);
-  const int ii = d == 0 ? gg : i, jj = d == 1 ? gg : j, kk = d == 2 ? gg : k;
-  return nflag[((size_t)kk * P.ny + jj) * P.nx + ii];
-}
-// interface f+1/2 along d (between nodes f and f+1) flagged?  (A6; the staggered wall plane never is)
-__device__ __forceinline__ int iface_flag(const DevP& P, const unsigned char* __restrict__ nflag, int d, int i, int j, int k, int f) {
-  const int n = d == 0 ? P.nx : (d == 1 ? P.ny : P.nz);
-  if ((f == -1 && P.bc[2 * d] == BC_WALL_STAG) || (f == n - 1 && P.bc[2 * d + 1] == BC_WALL_STAG)) return 0;
-  int any = 0;
-#pragma unroll
-  for (int g = -2; g <= 3; ++g) any |= nflag_at(P, nflag, d, i, j, k, f + g);
-  return any;
-}
-
 constexpr unsigned int IFACE_BELOW = 0x80000000u;      // interface-list entry: the interface BELOW the (first) node
 // offset of node (i,j,k) inside the boundary plane of direction D (scratch of the IFACE_BELOW entries)
 template <int D>
@@ -84,77 +67,167 @@ __device__ __forceinline__ size_t plane_base(const DevP& P) {
   return D == 0 ? 0 : (D == 1 ? 5 * plane_size<0>(P) : 5 * (plane_size<0>(P) + plane_size<1>(P)));
 }
 
-// list of nodes with a flagged interface; entry = node index, mask bit (2d+side), side 0 = below, 1 = above
-__global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P, const unsigned char* __restrict__ nflag,
+// ---- node flags as bits: fbits[row][wi], row = k * ny + j, bit b of word wi = node i = 32 wi + b (0 beyond nx) ----
+__device__ __forceinline__ int words_per_row(const DevP& P) { return (P.nx + 31) >> 5; }
+
+__global__ void __launch_bounds__(RT) k_flag_pack(const __grid_constant__ DevP P, const unsigned char* __restrict__ nflag,
+                                                  unsigned int* __restrict__ fbits) {
+  const int nw = words_per_row(P);
+  const unsigned int nwords = (unsigned int)(P.ny * P.nz) * (unsigned int)nw;
+  const int lane = threadIdx.x & 31;
+  for (unsigned int wd = (blockIdx.x * RT + threadIdx.x) >> 5; wd < nwords; wd += (gridDim.x * RT) >> 5) {
+    const unsigned int row = wd / (unsigned int)nw, wi = wd - row * (unsigned int)nw;
+    const int i = (int)(wi << 5) + lane;
+    const int f = i < P.nx ? nflag[(size_t)row * P.nx + i] : 0;
+    const unsigned int bits = __ballot_sync(0xffffffffu, f != 0);
+    if (lane == 0) fbits[wd] = bits;
+  }
+}
+
+// one node flag by (possibly ghost) x index of row `rw`: periodic wrap, else nearest interior node (A17)
+__device__ __forceinline__ unsigned int xbit(const DevP& P, const unsigned int* __restrict__ rw, int i) {
+  const int ii = P.bc[0] == BC_PERIODIC ? wrap(i, P.nx) : min(max(i, 0), P.nx - 1);
+  return (rw[ii >> 5] >> (ii & 31)) & 1u;
+}
+// row index of (j, k) with the ghost rule of the sensor along y / z
+__device__ __forceinline__ int row_of(const DevP& P, int j, int k) {
+  const int jj = P.bc[2] == BC_PERIODIC ? wrap(j, P.ny) : min(max(j, 0), P.ny - 1);
+  const int kk = P.bc[4] == BC_PERIODIC ? wrap(k, P.nz) : min(max(k, 0), P.nz - 1);
+  return kk * P.ny + jj;
+}
+
+// Interface flags and lists from the packed node flags, ONE THREAD PER WORD (32 nodes of a row): interface i+1/2 along
+// d is flagged iff any of nodes i-2..i+3 is (A6), i.e. an OR of six shifted words (x) or of six words of neighbouring
+// rows / planes (y, z).  Entries: node list (node index + 6-bit mask, bit 2d = interface below, 2d+1 = above) of the
+// nodes with a flagged interface, and per direction the list of flagged interfaces by their lower node (the interface
+// below the first node of a non-periodic direction: node | IFACE_BELOW).  A warp reserves its slots with one atomic
+// per list; inside a warp the entries follow the words, i.e. x, so that the consumers read their stencils coalesced.
+__global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P, const unsigned int* __restrict__ fbits,
                                                   unsigned int* __restrict__ list, unsigned char* __restrict__ lmask,
                                                   unsigned int* __restrict__ ilist /* [3][istride] or NULL */, size_t istride,
                                                   unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
+  const int nw = words_per_row(P);
+  const unsigned int nwords = (unsigned int)(P.ny * P.nz) * (unsigned int)nw;
+  const int lane = threadIdx.x & 31;
   unsigned long long cnt[3] = {0, 0, 0};
-  // every lane runs the same number of iterations (the ballot below needs the whole warp); lanes past the end idle
-  const long long nround = (P.N + (long long)gridDim.x * RT - 1) / ((long long)gridDim.x * RT);
-  for (long long it = 0; it < nround; ++it) {
-    const long long o = (it * gridDim.x + blockIdx.x) * (long long)RT + threadIdx.x;
-    const bool in = o < P.N;
-    // 32-bit index arithmetic: N < 2^31 with the hybrid switch on (validate())
-    const unsigned int o32 = in ? (unsigned int)o : 0u, row = o32 / (unsigned int)P.nx;
-    const int i = (int)(o32 - row * (unsigned int)P.nx), k = (int)(row / (unsigned int)P.ny), j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
-    const int id[3] = {i, j, k};
-    int mask = 0;
+  const unsigned int nround = (nwords + gridDim.x * RT - 1) / (gridDim.x * RT);
+  for (unsigned int it = 0; it < nround; ++it) {
+    const unsigned int wd = (it * gridDim.x + blockIdx.x) * RT + threadIdx.x;
+    const bool in = wd < nwords;
+    unsigned int lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    unsigned int row = 0, i0 = 0;
+    int j = 0, k = 0;
     if (in) {
+      row = wd / (unsigned int)nw;
+      const unsigned int wi = wd - row * (unsigned int)nw;
+      i0 = wi << 5;
+      k = (int)(row / (unsigned int)P.ny); j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
+      const int nvalid = min(32, P.nx - (int)i0);
+      const unsigned int valid = nvalid == 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
+      // ---- x: 38-bit window, bit b = node i0 - 3 + b
+      {
+        const unsigned int* rw = fbits + (size_t)row * nw;
+        unsigned long long V = (unsigned long long)rw[wi] << 3;
 #pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        // interfaces id-1/2 and id+1/2 look at nodes id-3..id+2 and id-2..id+3: one pass over the seven node flags
-        const int n = d == 0 ? P.nx : (d == 1 ? P.ny : P.nz);
-        int fl[7];
+        for (int b = 0; b < 3; ++b) V |= (unsigned long long)xbit(P, rw, (int)i0 - 3 + b) << b;
+        // nodes right of the word: the next word when it is whole inside the row, else bit by bit (row end, ghosts)
+        if ((int)i0 + 35 <= P.nx) V |= (unsigned long long)(rw[wi + 1] & 7u) << 35;
+        else {
 #pragma unroll
-        for (int g = 0; g < 7; ++g) fl[g] = nflag_at(P, nflag, d, i, j, k, id[d] - 3 + g);
-        int lo = fl[0] | fl[1] | fl[2] | fl[3] | fl[4] | fl[5];
-        int hi = fl[1] | fl[2] | fl[3] | fl[4] | fl[5] | fl[6];
-        if (id[d] == 0 && P.bc[2 * d] == BC_WALL_STAG) lo = 0;            // the staggered wall plane is never flagged (A6)
-        if (id[d] == n - 1 && P.bc[2 * d + 1] == BC_WALL_STAG) hi = 0;
-        mask |= (lo << (2 * d)) | (hi << (2 * d + 1));
-        cnt[d] += hi;
-        if (id[d] == 0 && P.bc[2 * d] != BC_PERIODIC) cnt[d] += lo;
-        if (iflags_out) iflags_out[d * P.N + o] = (unsigned char)hi;
+          for (int b = 0; b < 3; ++b) V |= (unsigned long long)xbit(P, rw, (int)i0 + 32 + b) << (35 + b);
+          // the word's own bits beyond nx hold 0: ghost nodes inside the word take the rule as well
+          for (int b = nvalid; b < min(32, nvalid + 3); ++b) V |= (unsigned long long)xbit(P, rw, (int)i0 + b) << (3 + b);
+        }
+        unsigned long long H = 0, L = 0;
+#pragma unroll
+        for (int sft = 1; sft <= 6; ++sft) H |= V >> sft;          // nodes i-2 .. i+3  <->  window bits n+1 .. n+6
+#pragma unroll
+        for (int sft = 0; sft <= 5; ++sft) L |= V >> sft;          // nodes i-3 .. i+2
+        hi[0] = (unsigned int)H & valid; lo[0] = (unsigned int)L & valid;
+      }
+      // ---- y and z: the same word of six neighbouring rows / planes
+      {
+        unsigned int wy[7], wz[7];
+#pragma unroll
+        for (int g = 0; g < 7; ++g) {
+          wy[g] = fbits[(size_t)row_of(P, j - 3 + g, k) * nw + wi];
+          wz[g] = fbits[(size_t)row_of(P, j, k - 3 + g) * nw + wi];
+        }
+        lo[1] = wy[0] | wy[1] | wy[2] | wy[3] | wy[4] | wy[5]; hi[1] = wy[1] | wy[2] | wy[3] | wy[4] | wy[5] | wy[6];
+        lo[2] = wz[0] | wz[1] | wz[2] | wz[3] | wz[4] | wz[5]; hi[2] = wz[1] | wz[2] | wz[3] | wz[4] | wz[5] | wz[6];
+      }
+      // the staggered wall plane is never flagged (A6)
+      if (P.bc[0] == BC_WALL_STAG && i0 == 0) lo[0] &= ~1u;
+      if (P.bc[1] == BC_WALL_STAG && (int)i0 + nvalid == P.nx) hi[0] &= ~(1u << (nvalid - 1));
+      if (P.bc[2] == BC_WALL_STAG && j == 0) lo[1] = 0;
+      if (P.bc[3] == BC_WALL_STAG && j == P.ny - 1) hi[1] = 0;
+      if (P.bc[4] == BC_WALL_STAG && k == 0) lo[2] = 0;
+      if (P.bc[5] == BC_WALL_STAG && k == P.nz - 1) hi[2] = 0;
+      cnt[0] += __popc(hi[0]) + ((i0 == 0 && P.bc[0] != BC_PERIODIC) ? (lo[0] & 1u) : 0u);
+      cnt[1] += __popc(hi[1]) + ((j == 0 && P.bc[2] != BC_PERIODIC) ? __popc(lo[1]) : 0);
+      cnt[2] += __popc(hi[2]) + ((k == 0 && P.bc[4] != BC_PERIODIC) ? __popc(lo[2]) : 0);
+      if (iflags_out) {
+        for (int b = 0; b < nvalid; ++b) {
+          const size_t o = (size_t)row * P.nx + i0 + b;
+#pragma unroll
+          for (int d = 0; d < 3; ++d) iflags_out[d * P.N + o] = (unsigned char)((hi[d] >> b) & 1u);
+        }
       }
     }
-    // warp-aggregated appends: the entries of a warp take consecutive slots in lane (= x) order, so that the
-    // consumers read their stencils coalesced
-    const int lane = threadIdx.x & 31;
+    const unsigned int o0 = row * (unsigned int)P.nx + i0;           // node of bit 0 (N < 2^31 with the switch on)
+    // ---- interface lists
     if (ilist) {
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        const bool hi = (mask >> (2 * d + 1)) & 1;
-        const unsigned int bd = __ballot_sync(0xffffffffu, hi);
-        if (bd) {
-          const int leader = __ffs(bd) - 1;
-          unsigned int base = 0;
-          if (lane == leader) base = atomicAdd(&sc->icount[d], (unsigned int)__popc(bd));
-          base = __shfl_sync(0xffffffffu, base, leader);
-          if (hi) ilist[d * istride + base + __popc(bd & ((1u << lane) - 1u))] = (unsigned int)o;
+        // below-entries: first node of a non-periodic direction
+        unsigned int lb = 0;
+        if (in && P.bc[2 * d] != BC_PERIODIC) {
+          if (d == 0) lb = i0 == 0 ? (lo[0] & 1u) : 0u;
+          else if (d == 1) lb = j == 0 ? lo[1] : 0u;
+          else lb = k == 0 ? lo[2] : 0u;
         }
-        // the interface between the ghost node and the first node of a non-periodic direction has no lower node:
-        // entry = first node | IFACE_BELOW (rare: one plane per direction; istride = N + the largest plane)
-        const bool lob = in && id[d] == 0 && P.bc[2 * d] != BC_PERIODIC && ((mask >> (2 * d)) & 1);
-        if (__any_sync(0xffffffffu, lob) && lob) ilist[d * istride + atomicAdd(&sc->icount[d], 1u)] = (unsigned int)o | IFACE_BELOW;
+        const unsigned int n_me = in ? (unsigned int)(__popc(hi[d]) + __popc(lb)) : 0u;
+        unsigned int pre = n_me;                                     // inclusive warp prefix sum
+#pragma unroll
+        for (int sft = 1; sft < 32; sft <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, pre, sft); if (lane >= sft) pre += t; }
+        const unsigned int tot = __shfl_sync(0xffffffffu, pre, 31);
+        unsigned int base = 0;
+        if (tot) {
+          if (lane == 31) base = atomicAdd(&sc->icount[d], tot);
+          base = __shfl_sync(0xffffffffu, base, 31);
+        }
+        unsigned int pos = base + pre - n_me;
+        unsigned int* li = ilist + d * istride;
+        for (unsigned int m = hi[d]; m; m &= m - 1) li[pos++] = o0 + (unsigned int)(__ffs(m) - 1);
+        for (unsigned int m = lb; m; m &= m - 1) li[pos++] = (o0 + (unsigned int)(__ffs(m) - 1)) | IFACE_BELOW;
       }
     }
-    const unsigned int bal = __ballot_sync(0xffffffffu, mask != 0 && list != nullptr);
-    if (bal) {
-      const int leader = __ffs(bal) - 1;
+    // ---- node list
+    if (list) {
+      const unsigned int any = in ? (lo[0] | hi[0] | lo[1] | hi[1] | lo[2] | hi[2]) : 0u;
+      const unsigned int n_me = (unsigned int)__popc(any);
+      unsigned int pre = n_me;
+#pragma unroll
+      for (int sft = 1; sft < 32; sft <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, pre, sft); if (lane >= sft) pre += t; }
+      const unsigned int tot = __shfl_sync(0xffffffffu, pre, 31);
       unsigned int base = 0;
-      if (lane == leader) base = atomicAdd(&sc->list_count, (unsigned int)__popc(bal));
-      base = __shfl_sync(0xffffffffu, base, leader);
-      if (mask && list) {
-        const unsigned int pos = base + __popc(bal & ((1u << lane) - 1u));
-        list[pos] = (unsigned int)o;
-        lmask[pos] = (unsigned char)mask;
+      if (tot) {
+        if (lane == 31) base = atomicAdd(&sc->list_count, tot);
+        base = __shfl_sync(0xffffffffu, base, 31);
+      }
+      unsigned int pos = base + pre - n_me;
+      for (unsigned int m = any; m; m &= m - 1) {
+        const int b = __ffs(m) - 1;
+        list[pos] = o0 + (unsigned int)b;
+        lmask[pos] = (unsigned char)(((lo[0] >> b) & 1u) | (((hi[0] >> b) & 1u) << 1) | (((lo[1] >> b) & 1u) << 2) |
+                                     (((hi[1] >> b) & 1u) << 3) | (((lo[2] >> b) & 1u) << 4) | (((hi[2] >> b) & 1u) << 5));
+        ++pos;
       }
     }
   }
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    for (int s = 16; s > 0; s >>= 1) cnt[d] += __shfl_down_sync(0xffffffffu, cnt[d], s);
+    for (int sft = 16; sft > 0; sft >>= 1) cnt[d] += __shfl_down_sync(0xffffffffu, cnt[d], sft);
     if ((threadIdx.x & 31) == 0 && cnt[d]) atomicAdd(&sc->weno_if[d], cnt[d]);
   }
 }
@@ -267,8 +340,8 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
 
 // one thread per listed interface of direction D: dF of the interface above node o -> dFbuf[D][v][o]
 // (IFACE_BELOW entries: the interface below the first node -> dFb, the boundary-plane scratch)
-template <int D>
-__global__ void __launch_bounds__(128) k_weno_flux(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ ilist,
+template <int D, int MB>
+__global__ void __launch_bounds__(128, MB) k_weno_flux(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ ilist,
                                                    size_t istride, const DevScal* __restrict__ sc, double* __restrict__ dFbuf, double* __restrict__ dFb) {
   const unsigned int n = sc->icount[D];
   const unsigned int* li = ilist + D * istride;
@@ -332,7 +405,9 @@ __global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP 
 #pragma unroll
         for (int v = 0; v < 5; ++v) dR[v] -= ih * dFbuf[o + v * P.N]; }
     }
-    {
+    // the characteristic forms at a non-reflecting top / characteristic wall replace the y-difference of those rows
+    const bool skip_y = (j == P.ny - 1 && P.bc[3] == BC_OUTFLOW) || (j == 0 && P.bc[2] == BC_WALL_CHAR);
+    if (!skip_y) {
       const double ih = P.ih[1][j];
       if (mask & 4) { dF_below<1>(P, dFbuf, dFb, i, j, k, dF);
 #pragma unroll
@@ -353,7 +428,7 @@ __global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP 
 #pragma unroll
     for (int v = 0; v < 5; ++v) R[o + v * P.N] += dR[v];
     if (q_new) {
-      const bool wall = (j == 0 && P.bc[2] == BC_WALL_NODE) || (j == P.ny - 1 && P.bc[3] == BC_WALL_NODE);
+      const bool wall = (j == 0 && node_wall(P.bc[2])) || (j == P.ny - 1 && node_wall(P.bc[3]));
       if (wall) {
         q_new[o] += dtb * dR[0];                      // u = v = w = 0 and T = T_w stay as overridden (S1)
       } else {

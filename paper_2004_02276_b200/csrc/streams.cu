@@ -35,6 +35,7 @@ struct streams_ctx {
   // workspace carve-up (caller memory)
   double *qbuf[2], *S[2], *theta, *partial, *inflow, *speeds;   // qbuf: primitives [NQ][N]; S: R registers [5][N]
   unsigned char *nflag, *lmask;
+  unsigned int* fbits;                 // node flags as bits, [nz*ny][ceil(nx/32)]
   unsigned int* list;
   unsigned int* ilist;                 // [3][N] interface lists (lower node of each flagged interface)
   double* dFbuf;                       // [3][5][N] dF of the interface above each node (flagged entries only)
@@ -128,10 +129,11 @@ const char* validate(const streams_grid* g, const streams_params* p) {
     if (lo == STREAMS_BC_PERIODIC && !(g->len[d] > 0.0)) return "periodic directions need len > 0";
     for (int s = 0; s < 2; ++s) {
       const int b = p->bc[2 * d + s];
-      if (b < 0 || b > STREAMS_BC_EXTRAP) return "unknown boundary kind";
+      if (b < 0 || b > STREAMS_BC_WALL_ISO_CHAR) return "unknown boundary kind";
+      if (b == STREAMS_BC_WALL_ISO_CHAR && !(d == 1 && s == 0)) return "WALL_ISO_CHAR is supported on ymin only";
       if ((b == STREAMS_BC_WALL_ISO_STAGGERED || b == STREAMS_BC_WALL_ISO_NODE) && d != 1) return "walls are supported on y faces only";
       if (b == STREAMS_BC_INFLOW_FROZEN && !(d == 0 && s == 0)) return "INFLOW_FROZEN is supported on xmin only";
-      if (b == STREAMS_BC_OUTFLOW_NR && !(d == 0 && s == 1)) return "OUTFLOW_NR is supported on xmax only";
+      if (b == STREAMS_BC_OUTFLOW_NR && !((d == 0 || d == 1) && s == 1)) return "OUTFLOW_NR is supported on xmax and ymax only";
       if (b == STREAMS_BC_SHOCKGEN && !(d == 1 && s == 1)) return "SHOCKGEN is supported on ymax only";
     }
   }
@@ -201,7 +203,7 @@ bool make_tile_map(CUtensorMap* tm, double* q, int nx, int ny, int nz) {
 
 struct Carve { size_t off = 0; size_t take(size_t bytes) { size_t o = off; off += up(bytes); return o; } };
 
-struct Layout { size_t w[2], S[2], theta, nflag, lmask, list, ilist, dFbuf, dFb, partial, inflow, speeds, total; int npartial; dim3 grid; int lz; size_t istride; };
+struct Layout { size_t w[2], S[2], theta, nflag, fbits, lmask, list, ilist, dFbuf, dFb, partial, inflow, speeds, total; int npartial; dim3 grid; int lz; size_t istride; };
 
 Layout make_layout(const streams_grid& g, const streams_params& p) {
   Layout L;
@@ -209,10 +211,11 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   Carve c;
   for (int i = 0; i < 2; ++i) L.w[i] = c.take(NQ * N * sizeof(double));
   for (int i = 0; i < 2; ++i) L.S[i] = c.take(5 * N * sizeof(double));
-  L.theta = L.nflag = L.lmask = L.list = L.ilist = L.dFbuf = L.dFb = 0;
+  L.theta = L.nflag = L.fbits = L.lmask = L.list = L.ilist = L.dFbuf = L.dFb = 0;
   if (p.weno_enable) {
     L.theta = c.take(N * sizeof(double));
     L.nflag = c.take(N);
+    L.fbits = c.take((size_t)g.ny * g.nz * ((g.nx + 31) / 32) * sizeof(unsigned int));
     L.lmask = c.take(N);
     L.list = c.take(N * sizeof(unsigned int));
     L.istride = N + std::max({(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny});
@@ -360,7 +363,7 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]); c->S[i] = (double*)(base + L.S[i]); }
   if (p->weno_enable) {
     c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
-    c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
+    c->fbits = (unsigned int*)(base + L.fbits); c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
     c->ilist = (unsigned int*)(base + L.ilist); c->dFbuf = (double*)(base + L.dFbuf); c->dFb = (double*)(base + L.dFb);
   }
   c->partial = (double*)(base + L.partial); c->inflow = (double*)(base + L.inflow); c->speeds = (double*)(base + L.speeds);
@@ -538,13 +541,21 @@ int streams_get_state_host(streams_ctx* c, double* h_w) {
   return STREAMS_OK;
 }
 
+// grid of the one-thread-per-flag-word list kernel
+static int wgrid_for(const streams_ctx* c) {
+  const long long words = (long long)c->P.ny * c->P.nz * ((c->P.nx + 31) / 32);
+  return (int)std::min<long long>(RGRID, (words + RT - 1) / RT);
+}
+
 // sensor + list of nodes with flagged interfaces for the state in `w`
 static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsigned char* iflags_out, bool build_list) {
   CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
   const int rg = rgrid_for(c->P.N);
   k_sensor<<<rg, RT, 0, c->st>>>(c->P, w, c->nflag, theta_out, c->sc);
   LAUNCH_CHECK("k_sensor");
-  k_weno_list<<<rg, RT, 0, c->st>>>(c->P, c->nflag, build_list ? c->list : nullptr, c->lmask, nullptr, 0, iflags_out, c->sc);
+  k_flag_pack<<<rg, RT, 0, c->st>>>(c->P, c->nflag, c->fbits);
+  LAUNCH_CHECK("k_flag_pack");
+  k_weno_list<<<wgrid_for(c), RT, 0, c->st>>>(c->P, c->fbits, build_list ? c->list : nullptr, c->lmask, nullptr, 0, iflags_out, c->sc);
   LAUNCH_CHECK("k_weno_list");
   return STREAMS_OK;
 }
@@ -553,7 +564,9 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
 static int run_list(streams_ctx* c) {
   CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
   CK(cudaMemsetAsync(&c->sc->icount[0], 0, 4 * sizeof(unsigned int), c->st));
-  k_weno_list<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->list, c->lmask, c->ilist, c->istride, nullptr, c->sc);
+  k_flag_pack<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->fbits);
+  LAUNCH_CHECK("k_flag_pack");
+  k_weno_list<<<wgrid_for(c), RT, 0, c->st>>>(c->P, c->fbits, c->list, c->lmask, c->ilist, c->istride, nullptr, c->sc);
   LAUNCH_CHECK("k_weno_list");
   return STREAMS_OK;
 }
@@ -563,11 +576,13 @@ static int run_list(streams_ctx* c) {
 static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, double beta) {
   int rc;
   if ((rc = run_list(c))) return rc;
-  k_weno_flux<0><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+  // 128 registers (4 CTAs of 128 threads per SM, 224 B of spills): 16 warps hide the fp64 latency of the reconstructions
+  // better than 232 registers at 8 warps (config 4, ms per RK3 step: 22.9 / 20.5 / 20.4 with 2 / 3 / 4 CTAs per SM)
+  k_weno_flux<0, 4><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
   LAUNCH_CHECK("k_weno_flux<0>");
-  k_weno_flux<1><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+  k_weno_flux<1, 4><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
   LAUNCH_CHECK("k_weno_flux<1>");
-  k_weno_flux<2><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+  k_weno_flux<2, 4><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
   LAUNCH_CHECK("k_weno_flux<2>");
   k_weno_apply<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->dFbuf, c->dFb, R, q_new, beta);
   LAUNCH_CHECK("k_weno_apply");

@@ -174,9 +174,13 @@ SMALL = {
     "channel_node_walls": lambda: mod(W.config3_channel(48, 24, 16), bc=NODE_WALLS),
     # the paper's own channel numerics: 4th order, Sutherland, error-function grid
     "channel_paper_small": lambda: W.config6_channel_paper(48, 24, 16),
+    # characteristic wall at the recovery temperature + non-reflecting top and outflow
+    "boundary_layer_small": lambda: W.config7_boundary_layer(64, 40, 8, Lx=12.0),
+    "boundary_layer_ragged": lambda: W.config7_boundary_layer(45, 30, 7, Lx=10.0),
+    "boundary_layer_weno": lambda: mod(W.config7_boundary_layer(45, 30, 7, Lx=10.0), weno_enable=1, sensor_threshold=-1.0),
 }
 
-STEPPED = ["channel_ragged", "channel_weno_forcing", "channel_node_walls", "sbli_weno_everywhere", "weno_mixed", "several_tiles_and_chunks"]
+STEPPED = ["boundary_layer_small", "boundary_layer_weno", "channel_paper_small", "channel_ragged", "channel_weno_forcing", "channel_node_walls", "sbli_weno_everywhere", "weno_mixed", "several_tiles_and_chunks"]
 
 
 @pytest.mark.parametrize("name", list(SMALL))
@@ -385,6 +389,14 @@ def test_config6_channel_paper_literal(env):
     check_rhs(env, wl)
     o, g, do, dg = check_steps(env, wl, wl.steps)
     assert abs(dg.forcing - do.forcing) <= 1e-9 * abs(do.forcing)
+
+
+def test_config7_boundary_layer(env):
+    """spatial boundary layer, M = 2, characteristic wall at T_r, non-reflecting
+    top and outflow, 256x64x32: one RHS and 20 RK3 steps against the oracle."""
+    wl = W.config7_boundary_layer()
+    check_rhs(env, wl)
+    check_steps(env, wl, wl.steps)
 
 
 def test_config3_channel(env):

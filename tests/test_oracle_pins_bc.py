@@ -450,3 +450,77 @@ def test_statistics_closed_form_plane_means(ob):
     assert np.abs(tau - 1.3 * 0.5 * (0.3 ** 2 + 0.5 ** 2) / 4).max() < 1e-14
     o.stats_reset()
     assert o.stats_read()[1] == 0 and np.abs(o.stats_read()[0]).max() == 0.0
+
+
+# ------------------------------------------------------------------ characteristic boundaries, PAPER.md:126 (8.f rank 3)
+def ycolumn(ob, ny, bc_lo, bc_hi, rho, v, p, u=None, Tw=1.0, visc=0):
+    y = np.arange(ny) / ny
+    bc = [W.BC_PERIODIC] * 2 + [bc_lo, bc_hi] + [W.BC_PERIODIC] * 2
+    prm = W.default_params(Rgas=R_GAS, viscous_enable=visc, T_wall=[Tw, Tw], bc=bc)
+    return column(ob, y, prm, rho, np.zeros(ny) if u is None else u, v, np.zeros(ny), p), y
+
+
+def test_characteristic_faces_reduce_to_the_LODI_relations(ob):
+    """Poinsot & Lele's locally one-dimensional inviscid relations in primitive variables, gas at rest plus a small
+    smooth perturbation (amplitude 1e-6: the conservative-variable form of S8 and the primitive form differ at second
+    order).  With L_1 = (v - c)(p_y - rho c v_y), L_5 = (v + c)(p_y + rho c v_y):
+      non-reflecting top (L_1 = 0):  rho_t = -L_5 / (2 c^2),  (rho v)_t = -L_5 / (2 c)    -> both from p_y + rho c v_y
+      reflecting wall (L_5 = L_1):   rho_t = -L_1 / c^2 = (p_y - rho c v_y) / c,  (rho v)_t = 0
+    with one-sided second-order differences at the boundary node."""
+    ny = 32
+    eps = 1e-6
+    yy = np.arange(ny) / ny
+    rho = 1.0 + eps * np.sin(3 * yy + 0.4)
+    v = eps * np.cos(2 * yy + 0.1)
+    v[0] = 0.0                                             # no slip at the wall node
+    p = 1.0 / GAM + eps * np.sin(5 * yy - 0.3)
+    o, y = ycolumn(ob, ny, W.BC_WALL_CHAR, W.BC_OUTFLOW, rho, v, p, Tw=float(p[0] / (R_GAS * rho[0])))
+    conv, _ = o.rhs_parts()
+    conv = conv[:, 0, :, 0]
+    h = 1.0 / ny
+    # top node: backward differences
+    py = (3 * p[-1] - 4 * p[-2] + p[-3]) / (2 * h)
+    vy = (3 * v[-1] - 4 * v[-2] + v[-3]) / (2 * h)
+    c_ = math.sqrt(GAM * p[-1] / rho[-1])
+    L5 = (v[-1] + c_) * (py + rho[-1] * c_ * vy)
+    assert abs(conv[0, -1] + L5 / (2 * c_ * c_)) < 1e-4 * abs(L5)
+    assert abs(conv[2, -1] + L5 / (2 * c_)) < 1e-4 * abs(L5)
+    # wall node: forward differences
+    py = (-3 * p[0] + 4 * p[1] - p[2]) / (2 * h)
+    vy = (-3 * v[0] + 4 * v[1] - v[2]) / (2 * h)
+    c_ = math.sqrt(GAM * p[0] / rho[0])
+    L1 = (v[0] - c_) * (py - rho[0] * c_ * vy)
+    assert abs(conv[0, 0] + L1 / (c_ * c_)) < 1e-4 * abs(L1)
+    assert abs(conv[2, 0]) < 1e-6 * abs(L1)
+    # a uniform state gives exactly zero at both faces
+    one = np.ones(ny)
+    o2, _ = ycolumn(ob, ny, W.BC_WALL_CHAR, W.BC_OUTFLOW, one, 0 * one, one / GAM)
+    assert np.abs(o2.rhs()).max() < 1e-13
+
+
+def run_pulse(ob, bc_lo, bc_hi, centre, direction, T_end, ny=96):
+    """Acoustic pulse of amplitude 1e-3 in gas at rest (rho = c = 1) running up (+1) or down (-1) the column."""
+    amp = 1e-3
+    yy = np.arange(ny) / ny
+    g = amp * np.exp(-((yy - centre) / 0.05) ** 2)
+    o, y = ycolumn(ob, ny, bc_lo, bc_hi, 1.0 + g, direction * g, 1.0 / GAM + g)
+    while o.diagnostics().time < T_end:
+        o.step(1)
+    w = o.get_state()[:, 0, :, 0]
+    return yy, w, amp
+
+
+def test_nonreflecting_top_lets_a_pulse_out(ob):
+    yy, w, amp = run_pulse(ob, W.BC_EXTRAP, W.BC_OUTFLOW, 0.7, +1, 0.6)
+    assert np.abs(w[0][8:] - 1.0).max() < 0.05 * amp                       # nothing comes back from the top
+
+
+def test_characteristic_wall_reflects_a_pulse(ob):
+    """A pulse running down to the characteristic wall comes back with the same sign and (nearly) the same amplitude,
+    the wall pressure peaks near twice the incident amplitude, and the wall row stays at rest (rigid, isothermal)."""
+    yy, w, amp = run_pulse(ob, W.BC_WALL_CHAR, W.BC_OUTFLOW, 0.3, -1, 0.6)
+    rho, v = w[0], w[2] / w[0]
+    k = int(np.argmax(np.abs(rho - 1.0)))
+    assert 0.2 < yy[k] < 0.4 and 0.85 * amp < rho[k] - 1.0 < 1.1 * amp       # back where it started, same sign
+    assert v[k] > 0.8 * amp                                                  # and now running upwards
+    assert w[2][0] == 0.0

@@ -14,7 +14,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-BC_PERIODIC, BC_WALL_STAG, BC_WALL_NODE, BC_INFLOW, BC_OUTFLOW, BC_SHOCKGEN, BC_EXTRAP = range(7)
+BC_PERIODIC, BC_WALL_STAG, BC_WALL_NODE, BC_INFLOW, BC_OUTFLOW, BC_SHOCKGEN, BC_EXTRAP, BC_WALL_CHAR = range(8)
 VISC_POWER, VISC_SUTHERLAND = 0, 1
 
 
@@ -296,8 +296,16 @@ def _similarity_profile(M, gamma, Pr, Tw, expo=0.76, eta_max=12.0, n=4801):
     return eta, yphys, fp, g
 
 
-def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0, Lz=4.0) -> Workload:
-    gamma, Pr, M = 1.4, 0.72, 2.28
+def config7_boundary_layer(nx=256, ny=64, nz=32, seed=1007, steps=20, Lx=24.0, Ly=8.0, Lz=4.0) -> Workload:
+    """Spatially developing supersonic boundary layer in the paper's set-up:
+    M_inf = 2, characteristic wave treatment at the no-slip wall at the recovery temperature, non-reflecting upper and
+    outflow boundaries, central flux only; the digital-filter inflow needs the database of ref. [40] (absent): frozen
+    laminar similarity inflow plus seeded fluctuations stand in for it."""
+    return config4_sbli(nx, ny, nz, seed, steps, Lx, Ly, Lz, M=2.0, shock=False, name="boundary_layer")
+
+
+def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0, Lz=4.0, M=2.28, shock=True, name="sbli") -> Workload:
+    gamma, Pr = 1.4, 0.72
     x = Lx * np.arange(nx) / (nx - 1.0)
     z = Lz * np.arange(nz) / nz
     y = sinh_nodes(ny, Ly)
@@ -307,6 +315,8 @@ def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0,
                             sensor_eps=(M / 1.0) ** 2, T_wall=[Tr, Tr], fs=[1.0, M, 0.0, 0.0, 1.0],
                             shock_angle_deg=8.0, x_shock=x_shock, cfl=0.5,
                             bc=[BC_INFLOW, BC_OUTFLOW, BC_WALL_NODE, BC_SHOCKGEN, BC_PERIODIC, BC_PERIODIC])
+    if not shock:
+        params.update(weno_enable=0, shock_angle_deg=0.0, bc=[BC_INFLOW, BC_OUTFLOW, BC_WALL_CHAR, BC_OUTFLOW, BC_PERIODIC, BC_PERIODIC])
     grid = dict(nx=nx, ny=ny, nz=nz, len=[Lx, Ly, Lz])
     cache = {}
 
@@ -336,7 +346,7 @@ def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0,
         pr_ = 1.0 + 2.0 * gamma / (gamma + 1.0) * (Mn * Mn - 1.0)
         rr_ = (gamma + 1.0) * Mn * Mn / ((gamma - 1.0) * Mn * Mn + 2.0)
         X, Y = np.meshgrid(x, y, indexing="xy")          # [ny][nx]
-        behind = (X - x_shock) > (Ly - Y) / np.tan(beta)
+        behind = ((X - x_shock) > (Ly - Y) / np.tan(beta)) & shock
         u = np.broadcast_to(u1[:, None], X.shape).copy()
         T = np.broadcast_to(T1[:, None], X.shape).copy()
         v = np.zeros_like(u)
@@ -371,7 +381,7 @@ def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0,
             w[i] += nz_[2] * env
         return prim_to_cons(rho, u, v, w, p, gamma)
 
-    return Workload("sbli", grid, x, y, z, params, steps, seed, state)
+    return Workload(name, grid, x, y, z, params, steps, seed, state)
 
 
 # ---------------------------------------------------------------------------------------------
