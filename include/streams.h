@@ -62,10 +62,14 @@ enum {
   STREAMS_BC_SHOCKGEN = 5,           /* inviscid oblique-shock state imposed in the ghosts of ymax
                                                                                  */
   STREAMS_BC_EXTRAP = 6,             /* zeroth-order extrapolation (1-D tube tests)            */
-  STREAMS_BC_WALL_ISO_CHAR = 7       /* ymin only: isothermal no-slip wall on the boundary node with the "similar
+  STREAMS_BC_WALL_ISO_CHAR = 7,      /* ymin only: isothermal no-slip wall on the boundary node with the "similar
                                         characteristic wave treatment" of PAPER.md:126: the wall-normal convective
                                         derivative at the wall node in characteristic form, incoming acoustic wave =
                                         reflection of the outgoing one (A14b)        */
+  STREAMS_BC_HALO = 8                /* zmin / zmax only: the face is an internal boundary of a domain decomposed into
+                                        z-slabs ("ghost nodes ... are exchanged between neighbouring
+                                        processes").  The three ghost planes beyond the face are STORED with the state and
+                                        filled by streams_halo_unpack; the context advances by the staged calls below */
 };
 
 enum { STREAMS_VISC_POWER = 0, STREAMS_VISC_SUTHERLAND = 1 };
@@ -128,7 +132,8 @@ size_t streams_workspace_bytes(const streams_grid* grid, const streams_params* p
  * the metrics of Eq. 5 generalised to non-uniform spacing, S2), gas model (Eq. 2-3),
  * scheme order, boundary kinds and forcing.
  * h_x/h_y/h_z: HOST arrays of nx/ny/nz node coordinates, strictly
- * increasing.  d_workspace: DEVICE memory, >= streams_workspace_bytes(), 256-B aligned,
+ * increasing.  A z face of kind BC_HALO adds the three node coordinates of the neighbouring slab on that side: h_z then
+ * holds [3 ghost coordinates if bc[zmin] == HALO][nz nodes][3 ghost coordinates if bc[zmax] == HALO], increasing.  d_workspace: DEVICE memory, >= streams_workspace_bytes(), 256-B aligned,
  * owned by the caller.  cuda_stream: cudaStream_t as void*.  On success *out is set. */
 int streams_create(const streams_grid* grid, const double* h_x, const double* h_y, const double* h_z,
                    const streams_params* params, void* d_workspace, size_t workspace_bytes,
@@ -164,6 +169,43 @@ int streams_sensor(streams_ctx* ctx, double* d_theta_out, unsigned char* d_flags
  * stage.  No host synchronisation.  On a stream of the caller's own (not the legacy default
  * stream) grids below 2^24 nodes replay one captured CUDA graph per step instead of launching kernel by kernel. */
 int streams_step(streams_ctx* ctx, int nsteps);
+
+/* ---- Staged stepping and z-slab halos: the domain decomposition of PAPER.md:168 and the overlapped ghost-node swap of
+ * PAPER.md:229-237 (section 4.3, Fig. 8), restricted to slabs along z (one slab per context / GPU; the caller moves the
+ * messages: NCCL, MPI or a device-to-device copy).  One RK3 step of Eq. 11 is
+ *     streams_step_begin                        local CFL maximum -> red[2]          [caller: MAX of red[2] over the slabs]
+ *     for stage = 0, 1, 2:
+ *         [caller: exchange the halos of the current state: pack / send / receive / unpack]
+ *         streams_stage_rhs(stage, part)        fused residual + stage kernel; body-force sums -> red[0], red[1]
+ *                                               [caller: SUM of red[0..1] over the slabs (forcing = 1 only)]
+ *         streams_stage_end(stage)              f = -red[0] / red[1], forcing fix, WENO correction, (stage 2) time += dt
+ * and gives bit for bit the state of streams_step when there is one slab (no BC_HALO face) and nothing is combined.
+ * `part`: STREAMS_PART_ALL launches the whole grid.  For overlap, STREAMS_PART_INTERIOR launches the z-chunks that read
+ * no ghost plane (possibly none on a thin slab) and may run while the halos are in flight; STREAMS_PART_BOUNDARY then
+ * launches the first and the last chunk and the reductions.  Calls out of this order return STREAMS_ESTATE.
+ * streams_step refuses a context with a BC_HALO face.  All calls are asynchronous on the context stream. */
+enum { STREAMS_PART_ALL = 0, STREAMS_PART_INTERIOR = 1, STREAMS_PART_BOUNDARY = 2 };
+int streams_step_begin(streams_ctx* ctx);
+int streams_stage_rhs(streams_ctx* ctx, int stage, int part);
+int streams_stage_end(streams_ctx* ctx, int stage);
+
+/* DEVICE pointer (inside the caller's workspace, valid for the life of the context) to four doubles:
+ *   red[0] = sum over the context's nodes of R_rhou vol, red[1] = sum of vol   (S9),
+ *   red[2] = max over nodes and directions of (|u_d| + c) / h_d                (S10), red[3] unused.
+ * The caller combines them across slabs in place (sum, sum, max) on the context stream between the staged calls. */
+double* streams_reduce_ptr(streams_ctx* ctx);
+
+/* Ghost-plane messages of the CURRENT state (the swap of the ghost nodes).  A message is the three planes
+ * next to a z face as stored primitives, [7][3][ny][nx] fp64 = streams_halo_bytes() bytes (rho, u, v, w, T, mu, H: sending
+ * mu and H as well saves the receiver a power law per ghost node and keeps slabs bit-identical to the undivided run).
+ * streams_halo_pack copies the INTERIOR planes next to `face` (4 = zmin: planes 0..2, 5 = zmax: planes nz-3..nz-1) into
+ * d_buf; streams_halo_unpack copies d_buf into the GHOST planes beyond `face` (which must be BC_HALO).  The message packed
+ * at the zmax face of slab r is what slab r+1 unpacks at its zmin face, and vice versa.  Device-to-device, asynchronous on
+ * `cuda_stream` (NULL = the context stream; another stream lets the swap overlap STREAMS_PART_INTERIOR, ordering between
+ * the two streams is the caller's: events). */
+size_t streams_halo_bytes(const streams_ctx* ctx);
+int streams_halo_pack(streams_ctx* ctx, int face, double* d_buf, void* cuda_stream);
+int streams_halo_unpack(streams_ctx* ctx, int face, const double* d_buf, void* cuda_stream);
 
 /* Reductions of the current state into *h_out (host struct): the volume integrals of PAPER.md:107 (bulk density
  * rho_b = 1/V int rho dV and bulk momentum, "both exactly constant in time"), total energy and kinetic energy

@@ -16,7 +16,8 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, S
 
 EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
-           "streams_diagnostics", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
+           "streams_diagnostics", "streams_step_begin", "streams_stage_rhs", "streams_stage_end", "streams_reduce_ptr",
+           "streams_halo_bytes", "streams_halo_pack", "streams_halo_unpack", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
 
 
 class StreamsGrid(C.Structure):
@@ -72,6 +73,15 @@ def lib():
         L.streams_sensor.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.streams_step.argtypes = [C.c_void_p, C.c_int]
         L.streams_diagnostics.argtypes = [C.c_void_p, C.POINTER(StreamsDiag)]
+        L.streams_step_begin.argtypes = [C.c_void_p]
+        L.streams_stage_rhs.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.streams_stage_end.argtypes = [C.c_void_p, C.c_int]
+        L.streams_reduce_ptr.argtypes = [C.c_void_p]
+        L.streams_reduce_ptr.restype = C.c_void_p
+        L.streams_halo_bytes.argtypes = [C.c_void_p]
+        L.streams_halo_bytes.restype = C.c_size_t
+        L.streams_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.streams_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.streams_stats_accumulate.argtypes = [C.c_void_p]
         L.streams_stats_read.argtypes = [C.c_void_p, _DBL, C.POINTER(C.c_longlong)]
         L.streams_stats_reset.argtypes = [C.c_void_p]
@@ -156,6 +166,7 @@ class Streams:
             raise StreamsError(rc, lib().streams_last_error(None).decode())
         self._h = h
         self.workspace_bytes = nbytes
+        self._red = None
 
     def close(self):
         if self._h:
@@ -256,6 +267,49 @@ class Streams:
 
     def step(self, n=1):
         self._chk(lib().streams_step(self._h, int(n)))
+
+    # --- staged stepping and z-slab halos (include/streams.h) ------------
+    PART_ALL, PART_INTERIOR, PART_BOUNDARY = 0, 1, 2
+    FACE_ZMIN, FACE_ZMAX = 4, 5
+
+    def step_begin(self):
+        self._chk(lib().streams_step_begin(self._h))
+
+    def stage_rhs(self, stage, part=0):
+        self._chk(lib().streams_stage_rhs(self._h, int(stage), int(part)))
+
+    def stage_end(self, stage):
+        self._chk(lib().streams_stage_end(self._h, int(stage)))
+
+    @property
+    def red(self):
+        """torch view (4 fp64, device) of the partial reductions the caller combines across slabs."""
+        if self._red is None:
+            ptr = lib().streams_reduce_ptr(self._h)
+            off = ptr - self._ws.data_ptr()
+            assert 0 <= off <= self.workspace_bytes - 32 and off % 8 == 0
+            self._red = self._ws[off:off + 32].view(self._torch.float64)
+        return self._red
+
+    def halo_shape(self):
+        return (7, 3, self.n[1], self.n[0])
+
+    def new_buffer(self):
+        """An uninitialised halo message buffer on the context's device."""
+        return self._torch.empty(self.halo_shape(), dtype=self._torch.float64, device=self.device)
+
+    def halo_pack(self, face, out=None, stream=None):
+        """Message [7][3][ny][nx] of the interior planes next to z face `face` (4 = zmin, 5 = zmax)."""
+        torch = self._torch
+        if out is None:
+            out = torch.empty(self.halo_shape(), dtype=torch.float64, device=self.device)
+        st = stream.cuda_stream if stream is not None else 0
+        self._chk(lib().streams_halo_pack(self._h, int(face), self._dev(out, self.halo_shape()), C.c_void_p(st)))
+        return out
+
+    def halo_unpack(self, face, buf, stream=None):
+        st = stream.cuda_stream if stream is not None else 0
+        self._chk(lib().streams_halo_unpack(self._h, int(face), self._dev(buf, self.halo_shape()), C.c_void_p(st)))
 
     def diagnostics(self, check=True):
         d = StreamsDiag()

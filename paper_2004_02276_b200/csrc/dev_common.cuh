@@ -18,7 +18,7 @@ namespace streams {
 constexpr int HALO = 3;
 constexpr int NQ = 7;                 // stored primitives per node
 
-enum { BC_PERIODIC = 0, BC_WALL_STAG = 1, BC_WALL_NODE = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_SHOCKGEN = 5, BC_EXTRAP = 6, BC_WALL_CHAR = 7 };
+enum { BC_PERIODIC = 0, BC_WALL_STAG = 1, BC_WALL_NODE = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_SHOCKGEN = 5, BC_EXTRAP = 6, BC_WALL_CHAR = 7, BC_HALO = 8 };
 enum { VISC_POWER = 0, VISC_SUTH = 1 };
 
 // central coefficients of order 2L, zero-padded to three entries
@@ -34,6 +34,9 @@ struct DevP {
   int bc[6];
   int visc_model, weno, forcing, viscous, L;
   long long N;                       // nx*ny*nz
+  long long QS;                      // doubles between two fields of a primitive-state buffer: (nz + 2 zpad) * nxy
+  int zpad;                          // ghost planes stored below / above the state (3 when a z face is BC_HALO, else 0)
+  int pad_;
   double gam, gm1, Rgas, inv_R, cp, cv, inv_cv, cp_over_Pr;
   double mu_ref, T_ref, inv_Tref, visc_exp, suth_S;
   double th_thr, th_eps;
@@ -146,9 +149,11 @@ __device__ __forceinline__ int map_y(const DevP& P, int j, int& mode) {
   }
   return j;
 }
+// z: plane index relative to the first interior plane.  A BC_HALO face keeps the index (-3..-1, nz..nz+2): those planes
+// are STORED around the state (DevP::zpad) and filled by streams_halo_unpack with the neighbouring slab's planes.
 __device__ __forceinline__ int map_z(const DevP& P, int k) {
-  if (k < 0) return P.bc[4] == BC_PERIODIC ? wrap(k, P.nz) : 0;
-  if (k >= P.nz) return P.bc[5] == BC_PERIODIC ? wrap(k, P.nz) : P.nz - 1;
+  if (k < 0) return P.bc[4] == BC_PERIODIC ? wrap(k, P.nz) : (P.bc[4] == BC_HALO ? k : 0);
+  if (k >= P.nz) return P.bc[5] == BC_PERIODIC ? wrap(k, P.nz) : (P.bc[5] == BC_HALO ? k : P.nz - 1);
   return k;
 }
 
@@ -191,9 +196,9 @@ __device__ __forceinline__ void reflect(const DevP& P, double Tw, Prim& q) {
 __device__ __forceinline__ void load_src_raw(const DevP& P, const double* __restrict__ Q, const Src s, int kk, Prim& q) {
   const int k = s.kind & 7;
   if (k == SRC_FIELD) {
-    const size_t o = (size_t)kk * P.nxy + s.off;
-    q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.N); q.v = __ldg(Q + o + 2 * P.N); q.w = __ldg(Q + o + 3 * P.N);
-    q.T = __ldg(Q + o + 4 * P.N); q.mu = __ldg(Q + o + 5 * P.N); q.H = __ldg(Q + o + 6 * P.N);
+    const long long o = (long long)kk * P.nxy + s.off;
+    q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.QS); q.v = __ldg(Q + o + 2 * P.QS); q.w = __ldg(Q + o + 3 * P.QS);
+    q.T = __ldg(Q + o + 4 * P.QS); q.mu = __ldg(Q + o + 5 * P.QS); q.H = __ldg(Q + o + 6 * P.QS);
   } else if (k == SRC_INFLOW) {
     const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
     q.rho = P.inflow[o]; q.u = P.inflow[o + st]; q.v = P.inflow[o + 2 * st]; q.w = P.inflow[o + 3 * st];
@@ -219,8 +224,8 @@ __device__ __forceinline__ void fetch_prim5(const DevP& P, const double* __restr
   const Src s = resolve_xy(P, i, j);
   const int kk = map_z(P, k), kd = s.kind & 7;
   if (kd == SRC_FIELD) {
-    const size_t o = (size_t)kk * P.nxy + s.off;
-    q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.N); q.v = __ldg(Q + o + 2 * P.N); q.w = __ldg(Q + o + 3 * P.N); q.T = __ldg(Q + o + 4 * P.N);
+    const long long o = (long long)kk * P.nxy + s.off;
+    q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.QS); q.v = __ldg(Q + o + 2 * P.QS); q.w = __ldg(Q + o + 3 * P.QS); q.T = __ldg(Q + o + 4 * P.QS);
   } else if (kd == SRC_INFLOW) {
     const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
     q.rho = P.inflow[o]; q.u = P.inflow[o + st]; q.v = P.inflow[o + 2 * st]; q.w = P.inflow[o + 3 * st]; q.T = P.inflow[o + 4 * st];
@@ -241,8 +246,8 @@ __device__ __forceinline__ void fetch_vel(const DevP& P, const double* __restric
   const Src s = resolve_xy(P, i, j);
   const int kk = map_z(P, k), kd = s.kind & 7;
   if (kd == SRC_FIELD) {
-    const size_t o = (size_t)kk * P.nxy + s.off;
-    u = __ldg(Q + o + P.N); v = __ldg(Q + o + 2 * P.N); w = __ldg(Q + o + 3 * P.N);
+    const long long o = (long long)kk * P.nxy + s.off;
+    u = __ldg(Q + o + P.QS); v = __ldg(Q + o + 2 * P.QS); w = __ldg(Q + o + 3 * P.QS);
   } else if (kd == SRC_INFLOW) {
     const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
     u = P.inflow[o + st]; v = P.inflow[o + 2 * st]; w = P.inflow[o + 3 * st];

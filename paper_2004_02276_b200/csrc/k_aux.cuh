@@ -24,9 +24,12 @@ struct DevScal {
   unsigned long long weno_if[3];
   unsigned int list_count;
   unsigned int pad;
-  double dt_next;       // S10 evaluated on the state at the end of a step (fused into the last k_force_fix)
   unsigned int icount[3];   // entries of the three interface lists (k_weno_list)
   unsigned int pad2;
+  // Partial reductions of THIS context, combined across z-slabs by the caller between the staged calls
+  // (include/streams.h, streams_reduce_ptr): red[0] = sum R_rhou vol, red[1] = sum vol  (S9: f = -red[0] / red[1]),
+  // red[2] = max over nodes and directions of (|u_d| + c) / h_d  (S10: dt = cfl / red[2]).
+  double red[4];
 };
 
 // ---- S3: conservative w[5][N] -> primitives Q[NQ][N]  (streams_set_state) ----
@@ -34,14 +37,14 @@ __global__ void __launch_bounds__(RT) k_cons2prim(const __grid_constant__ DevP P
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     Prim q;
     cons2prim(P, w[o], w[o + P.N], w[o + 2 * P.N], w[o + 3 * P.N], w[o + 4 * P.N], q);
-    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu; Q[o + 6 * P.N] = q.H;
+    Q[o] = q.rho; Q[o + P.QS] = q.u; Q[o + 2 * P.QS] = q.v; Q[o + 3 * P.QS] = q.w; Q[o + 4 * P.QS] = q.T; Q[o + 5 * P.QS] = q.mu; Q[o + 6 * P.QS] = q.H;
   }
 }
 // ---- primitives -> conservative (streams_get_state) ----
 __global__ void __launch_bounds__(RT) k_prim2cons(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ w) {
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     Prim q;
-    q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
+    q.rho = Q[o]; q.u = Q[o + P.QS]; q.v = Q[o + 2 * P.QS]; q.w = Q[o + 3 * P.QS]; q.T = Q[o + 4 * P.QS]; q.mu = 0.0;
     double wv[5];
     prim2cons(P, q, wv);
 #pragma unroll
@@ -58,7 +61,7 @@ __global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, d
   const double f = use_force ? sc->force : 0.0;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     Prim q;
-    q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
+    q.rho = Q[o]; q.u = Q[o + P.QS]; q.v = Q[o + 2 * P.QS]; q.w = Q[o + 3 * P.QS]; q.T = Q[o + 4 * P.QS]; q.mu = 0.0;
     double r[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) r[v] = Sc[o + v * P.N];
@@ -77,7 +80,7 @@ __global__ void __launch_bounds__(RT) k_update(const __grid_constant__ DevP P, d
     node_ijk(P, o, i_, j, k_);
     if (j == 0 && node_wall(P.bc[2])) wall_node_override(P, P.Twall[0], P.mu_wall[0], q);
     if (j == P.ny - 1 && node_wall(P.bc[3])) wall_node_override(P, P.Twall[1], P.mu_wall[1], q);
-    Q[o] = q.rho; Q[o + P.N] = q.u; Q[o + 2 * P.N] = q.v; Q[o + 3 * P.N] = q.w; Q[o + 4 * P.N] = q.T; Q[o + 5 * P.N] = q.mu; Q[o + 6 * P.N] = q.H;
+    Q[o] = q.rho; Q[o + P.QS] = q.u; Q[o + 2 * P.QS] = q.v; Q[o + 3 * P.QS] = q.w; Q[o + 4 * P.QS] = q.T; Q[o + 5 * P.QS] = q.mu; Q[o + 6 * P.QS] = q.H;
   }
 }
 
@@ -107,9 +110,9 @@ __global__ void __launch_bounds__(RT) k_force_fix(const __grid_constant__ DevP P
         const int i = ib + e * RT;
         if (i < P.nx) {
           const size_t o = r0 + i;
-          u[e] = Q[o + P.N]; T[e] = Q[o + 4 * P.N];
-          if (!wallrow) { rho[e] = Q[o]; H[e] = Q[o + 6 * P.N]; ul[e] = Qin[o + P.N]; }
-          if (speed) { vv[e] = Q[o + 2 * P.N]; ww[e] = Q[o + 3 * P.N]; }
+          u[e] = Q[o + P.QS]; T[e] = Q[o + 4 * P.QS];
+          if (!wallrow) { rho[e] = Q[o]; H[e] = Q[o + 6 * P.QS]; ul[e] = Qin[o + P.QS]; }
+          if (speed) { vv[e] = Q[o + 2 * P.QS]; ww[e] = Q[o + 3 * P.QS]; }
         }
       }
 #pragma unroll
@@ -125,8 +128,8 @@ __global__ void __launch_bounds__(RT) k_force_fix(const __grid_constant__ DevP P
             const double dke = 0.5 * (du * (un + u[e]));
             const double dT = (dE - dke) * P.inv_cv;
             Tn = T[e] + dT;
-            Q[o + P.N] = un; Q[o + 4 * P.N] = Tn; Q[o + 5 * P.N] = visc_mu(P, Tn);
-            Q[o + 6 * P.N] = H[e] + fma(P.cp, dT, dke);
+            Q[o + P.QS] = un; Q[o + 4 * P.QS] = Tn; Q[o + 5 * P.QS] = visc_mu(P, Tn);
+            Q[o + 6 * P.QS] = H[e] + fma(P.cp, dT, dke);
           }
           if (speed) {
             const double cs = sqrt(P.gam * P.Rgas * Tn);
@@ -151,7 +154,7 @@ __global__ void __launch_bounds__(RT) k_apply_force(const __grid_constant__ DevP
   const double f = sc->force;
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     R[o + 1 * P.N] += f;
-    R[o + 4 * P.N] = fma(f, Q[o + P.N], R[o + 4 * P.N]);
+    R[o + 4 * P.N] = fma(f, Q[o + P.QS], R[o + 4 * P.N]);
   }
 }
 
@@ -167,14 +170,19 @@ __global__ void __launch_bounds__(RT) k_force_partial(const __grid_constant__ De
   const double t = block_sum<RT>(acc, sh, threadIdx.x);
   if (threadIdx.x == 0) partial[blockIdx.x] = t;
 }
-// f = - sum(partials) / sum(vol), fixed summation order (one CTA)
-__global__ void __launch_bounds__(RT) k_force_final(const double* __restrict__ partial, int n, DevScal* sc) {
+// red[0] = sum(partials), red[1] = sum(vol), fixed summation order (one CTA); take != 0: f = - red[0] / red[1] at once
+// (single context; z-slabs combine red across contexts first and then run k_force_take)
+__global__ void __launch_bounds__(RT) k_force_final(const double* __restrict__ partial, int n, DevScal* sc, int take) {
   __shared__ double sh[RT / 32];
   double acc = 0.0;
   for (int e = threadIdx.x; e < n; e += RT) acc += partial[e];
   const double t = block_sum<RT>(acc, sh, threadIdx.x);
-  if (threadIdx.x == 0) sc->force = -t / sc->vol_total;
+  if (threadIdx.x == 0) {
+    sc->red[0] = t; sc->red[1] = sc->vol_total;
+    if (take) sc->force = -t / sc->vol_total;
+  }
 }
+__global__ void k_force_take(DevScal* sc) { sc->force = -sc->red[0] / sc->red[1]; }
 
 // ---- S10: dt = cfl / max_d max_nodes (|u_d| + c) / h_d ----
 __global__ void __launch_bounds__(RT) k_speed_partial(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ partial /*[3][grid]*/) {
@@ -183,18 +191,18 @@ __global__ void __launch_bounds__(RT) k_speed_partial(const __grid_constant__ De
   for (long long o = blockIdx.x * (long long)RT + threadIdx.x; o < P.N; o += (long long)gridDim.x * RT) {
     int i, j, k;
     node_ijk(P, o, i, j, k);
-    const double cs = sqrt(P.gam * P.Rgas * Q[o + 4 * P.N]);
-    m[0] = fmax(m[0], (fabs(Q[o + P.N]) + cs) * P.ih[0][i]);
-    m[1] = fmax(m[1], (fabs(Q[o + 2 * P.N]) + cs) * P.ih[1][j]);
-    m[2] = fmax(m[2], (fabs(Q[o + 3 * P.N]) + cs) * P.ih[2][k]);
+    const double cs = sqrt(P.gam * P.Rgas * Q[o + 4 * P.QS]);
+    m[0] = fmax(m[0], (fabs(Q[o + P.QS]) + cs) * P.ih[0][i]);
+    m[1] = fmax(m[1], (fabs(Q[o + 2 * P.QS]) + cs) * P.ih[1][j]);
+    m[2] = fmax(m[2], (fabs(Q[o + 3 * P.QS]) + cs) * P.ih[2][k]);
   }
   for (int d = 0; d < 3; ++d) {
     const double t = block_max<RT>(m[d], sh, threadIdx.x);
     if (threadIdx.x == 0) partial[d * gridDim.x + blockIdx.x] = t;
   }
 }
-__global__ void __launch_bounds__(RT) k_dt_final(const double* __restrict__ partial, int n, double cfl, double dt_fixed,
-                                                 DevScal* sc, double* __restrict__ speeds_out /* 3, may be NULL */, int set_dt) {
+__global__ void __launch_bounds__(RT) k_dt_final(const double* __restrict__ partial, int n, DevScal* sc,
+                                                 double* __restrict__ speeds_out /* 3, may be NULL */, int set_red) {
   __shared__ double sh[RT / 32];
   double mm = 0.0;
   for (int d = 0; d < 3; ++d) {
@@ -203,11 +211,11 @@ __global__ void __launch_bounds__(RT) k_dt_final(const double* __restrict__ part
     const double t = block_max<RT>(m, sh, threadIdx.x);
     if (threadIdx.x == 0) { mm = fmax(mm, t); if (speeds_out) speeds_out[d] = t; }
   }
-  if (threadIdx.x == 0 && set_dt == 1) sc->dt = dt_fixed > 0.0 ? dt_fixed : cfl / mm;
-  if (threadIdx.x == 0 && set_dt == 2) sc->dt_next = dt_fixed > 0.0 ? dt_fixed : cfl / mm;
+  if (threadIdx.x == 0 && set_red) sc->red[2] = mm;             // local maximum; k_take_dt turns it into the time step
 }
 __global__ void k_advance_time(DevScal* sc) { sc->time += sc->dt; }
-__global__ void k_take_dt(DevScal* sc) { sc->dt = sc->dt_next; }
+// S10: dt = cfl / max (|u_d| + c) / h_d, the maximum taken over the whole domain (red[2], combined across z-slabs)
+__global__ void k_take_dt(DevScal* sc, double cfl) { sc->dt = cfl / sc->red[2]; }
 
 // ---- diagnostics: per-block partials, reduced on the host by streams_diagnostics ----
 constexpr int NDIAG = 12;   // mass, mx, my, mz, E, ke, vol | min rho, min p, max Mach | nonfinite | spare
@@ -220,7 +228,7 @@ __global__ void __launch_bounds__(RT) k_diag_partial(const __grid_constant__ Dev
     node_ijk(P, o, i, j, k);
     const double vol = P.hh[0][i] * P.hh[1][j] * P.hh[2][k];
     Prim q;
-    q.rho = Q[o]; q.u = Q[o + P.N]; q.v = Q[o + 2 * P.N]; q.w = Q[o + 3 * P.N]; q.T = Q[o + 4 * P.N]; q.mu = 0.0;
+    q.rho = Q[o]; q.u = Q[o + P.QS]; q.v = Q[o + 2 * P.QS]; q.w = Q[o + 3 * P.QS]; q.T = Q[o + 4 * P.QS]; q.mu = 0.0;
     double wv[5];
     prim2cons(P, q, wv);
     const double q2 = q.u * q.u + q.v * q.v + q.w * q.w;
@@ -262,7 +270,7 @@ __global__ void k_capture_inflow(const __grid_constant__ DevP P, const double* _
   for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < NQ * n; e += (long long)gridDim.x * blockDim.x) {
     const int v = (int)(e / n);
     const long long r = e % n;
-    inflow[e] = Q[v * P.N + r * P.nx];
+    inflow[e] = Q[v * P.QS + r * P.nx];
   }
 }
 

@@ -85,6 +85,8 @@ struct RhsArgs {
                           // gradients; [N] bytes, NULL when the WENO switch is off
   double* partial;        // per-CTA partial sums of R_rhou * vol (forcing), may be NULL
   int lz;                 // planes per CTA
+  int cz0, czs;           // chunk of CTA z-index c is cz0 + c * czs (whole grid: 0, 1; streams_stage_rhs launches the chunks
+                          // that need no ghost plane of a BC_HALO face and the two boundary chunks separately)
   int use_tma;            // 1: tile by TMA box copies (tensor map over q); 0: every slot by index (odd nx)
 };
 
@@ -416,7 +418,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       for (int b = 0; b < 2; ++b)
         if (b < nplanes) {
           mbar_expect_tx(bar0 + 8 * b, TILE_BYTES);
-          tma_tile(smem_u32(tiles + b * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, k0 - 3 + b), bar0 + 8 * b);
+          tma_tile(smem_u32(tiles + b * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, k0 - 3 + b) + P.zpad, bar0 + 8 * b);
         }
     }
   }
@@ -455,9 +457,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   if (active) {
 #pragma unroll
     for (int a = 3; a < 6; ++a) {          // planes k0-3 .. k0-1 sit in slots 3..5 at s = k0-3
-      const double* q = A.q + own_off + (size_t)map_z(P, k0 - 6 + a) * P.nxy;
-      rw[a] = __ldg(q); uw[a] = __ldg(q + P.N); vw[a] = __ldg(q + 2 * P.N); ww[a] = __ldg(q + 3 * P.N);
-      Tw[a] = __ldg(q + 4 * P.N); mw[a] = __ldg(q + 5 * P.N); Hw[a] = __ldg(q + 6 * P.N);
+      const double* q = A.q + own_off + (long long)map_z(P, k0 - 6 + a) * P.nxy;
+      rw[a] = __ldg(q); uw[a] = __ldg(q + P.QS); vw[a] = __ldg(q + 2 * P.QS); ww[a] = __ldg(q + 3 * P.QS);
+      Tw[a] = __ldg(q + 4 * P.QS); mw[a] = __ldg(q + 5 * P.QS); Hw[a] = __ldg(q + 6 * P.QS);
     }
   }
   // own node of the planes ahead: plane s+5 is requested at the top of step s (cp.async, thread-private
@@ -465,9 +467,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 #pragma unroll
   for (int b = 0; b < 2; ++b) {
     if (active) {
-      const double* q = A.q + own_off + (size_t)map_z(P, k0 + b) * P.nxy;
+      const double* q = A.q + own_off + (long long)map_z(P, k0 + b) * P.nxy;
 #pragma unroll
-      for (int f = 0; f < NF; ++f) cp_async8(smem_u32(oring + tid) + ((b * NF + f) * NPT) * 8, q + f * P.N);
+      for (int f = 0; f < NF; ++f) cp_async8(smem_u32(oring + tid) + ((b * NF + f) * NPT) * 8, q + f * P.QS);
     }
     cp_async_commit();
   }
@@ -486,10 +488,10 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     const unsigned phase = (unsigned)(it >> 1) & 1u;
     double* t = tiles + buf * SM_TILE1;
     if (active && s + 5 < k1 + 3) {
-      const double* q = A.q + own_off + (size_t)map_z(P, s + 5) * P.nxy;
+      const double* q = A.q + own_off + (long long)map_z(P, s + 5) * P.nxy;
       const unsigned d = smem_u32(oring + tid) + ((b3 == 0 ? 2 : b3 - 1) * NF * NPT) * 8;       // (it + 5) % 3
 #pragma unroll
-      for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.N);
+      for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.QS);
     }
     if (FUSED && A.alpha != 0.0 && active && s - 2 >= k0 && s - 2 < k1) {
       // R_prev (and u_prev for the lazy forcing) of plane s-2, read in the NEXT step's epilogue (one step of slack:
@@ -498,7 +500,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       const unsigned d = smem_u32(spring + tid) + (((it + 1) & 1) * 6 * NPT) * 8;
 #pragma unroll
       for (int v = 0; v < 5; ++v) cp_async8(d + v * NPT * 8, A.S_prev + o + v * P.N);
-      if (A.f_prev) cp_async8(d + 5 * NPT * 8, A.q_out + o + P.N);
+      if (A.f_prev) cp_async8(d + 5 * NPT * 8, A.q_out + o + P.QS);
     }
     cp_async_commit();
     cp_async_wait<1>();                                  // the groups of steps <= s-1 have landed: own node of plane s+3
@@ -568,7 +570,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         double* gr = gring + slot7 * 3 * NPT + tl;
         gr[0] = d1_tile(P, t + F_W * TILE, loc, 1) * ihx;
         gr[NPT] = d1_tile(P, t + F_W * TILE, loc, PITCH) * ihy;
-        gr[2 * NPT] = dxu * ihx + dyv * ihy;
+        gr[2 * NPT] = __dadd_rn(__dmul_rn(dxu, ihx), __dmul_rn(dyv, ihy));   // = G[0] + G[4] of a full plane, bit for bit
       }
     } else {
       const double ihx = xi[li], ihy = yi[lj];
@@ -623,7 +625,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         }
       }
       double* gr = gring + slot7 * 3 * NPT + tl;
-      gr[0] = N.G[6]; gr[NPT] = N.G[7]; gr[2 * NPT] = N.G[0] + N.G[4];
+      // no FMA contraction here: a plane next to a chunk is a ghost plane of that chunk (branch above) and must give
+      // the same bits, so that the result does not depend on how z is cut into chunks or slabs
+      gr[0] = N.G[6]; gr[NPT] = N.G[7]; gr[2 * NPT] = __dadd_rn(N.G[0], N.G[4]);
     }
     // ---- the plane's barrier, first half: everything other threads read of this step is written ----
     __syncwarp();
@@ -702,9 +706,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         advance_prim<!LAZY>(P, qn, dW);
         if (!PLAIN && gj == 0 && node_wall(P.bc[2])) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
         if (!PLAIN && gj == P.ny - 1 && node_wall(P.bc[3])) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
-        A.q_out[o] = qn.rho; A.q_out[o + P.N] = qn.u; A.q_out[o + 2 * P.N] = qn.v; A.q_out[o + 3 * P.N] = qn.w;
-        A.q_out[o + 4 * P.N] = qn.T; A.q_out[o + 6 * P.N] = qn.H;
-        if (store_mu) A.q_out[o + 5 * P.N] = qn.mu;
+        A.q_out[o] = qn.rho; A.q_out[o + P.QS] = qn.u; A.q_out[o + 2 * P.QS] = qn.v; A.q_out[o + 3 * P.QS] = qn.w;
+        A.q_out[o + 4 * P.QS] = qn.T; A.q_out[o + 6 * P.QS] = qn.H;
+        if (store_mu) A.q_out[o + 5 * P.QS] = qn.mu;
       }
     }
     // ---- second half of the barrier: the staging rows of this plane are complete ----
@@ -714,7 +718,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       const int b2 = buf;                                // (it + 2) % NBUF
       fence_proxy_async();
       mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
-      tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2), bar0 + 8 * b2);
+      tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2) + P.zpad, bar0 + 8 * b2);
     }
     // ================= after the barrier: the xy mixed terms of plane s (A8), d_x(d_y v) and d_y(d_x u) from the
     // staging rows; they enter V_0, V_1 times mu / 3 and the viscous work u V_0 + v V_1.  R of plane s goes to the
@@ -762,7 +766,7 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   // march through different z ranges (spreads the DRAM traffic; one wave in lockstep through z measured 24 % slower)
   const int lin = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
   const int tix = lin / gridDim.z;
-  const int3 cta = make_int3(tix % gridDim.x, tix / gridDim.x, lin % gridDim.z);
+  const int3 cta = make_int3(tix % gridDim.x, tix / gridDim.x, A.cz0 + (lin % gridDim.z) * A.czs);
   const int i0 = cta.x * TX, j0 = cta.y * TY;
   const bool inside = i0 + TX <= P.nx && j0 + TY <= P.ny;
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;

@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(RT) k_stats_partial(const __grid_constant__ De
     const size_t r0 = ((size_t)k * P.ny + j) * P.nx;
     for (int i = threadIdx.x; i < P.nx; i += RT) {
       const size_t o = r0 + i;
-      const double rho = Q[o], u = Q[o + P.N], v = Q[o + 2 * P.N], w = Q[o + 3 * P.N], T = Q[o + 4 * P.N], mu = Q[o + 5 * P.N];
+      const double rho = Q[o], u = Q[o + P.QS], v = Q[o + 2 * P.QS], w = Q[o + 3 * P.QS], T = Q[o + 4 * P.QS], mu = Q[o + 5 * P.QS];
       const double ru = rho * u, rv = rho * v, rw = rho * w;
       a[0] += rho; a[1] += u; a[2] += v; a[3] += w; a[4] += rho * (P.Rgas * T); a[5] += T; a[6] += mu;
       a[7] += ru; a[8] += rv; a[9] += rw; a[10] += rho * T;

@@ -433,12 +433,12 @@ __global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP 
         q_new[o] += dtb * dR[0];                      // u = v = w = 0 and T = T_w stay as overridden (S1)
       } else {
         Prim q;
-        q.rho = q_new[o]; q.u = q_new[o + P.N]; q.v = q_new[o + 2 * P.N]; q.w = q_new[o + 3 * P.N]; q.T = q_new[o + 4 * P.N]; q.mu = 0.0;
+        q.rho = q_new[o]; q.u = q_new[o + P.QS]; q.v = q_new[o + 2 * P.QS]; q.w = q_new[o + 3 * P.QS]; q.T = q_new[o + 4 * P.QS]; q.mu = 0.0;
         double dW[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) dW[v] = dtb * dR[v];
         advance_prim(P, q, dW);
-        q_new[o] = q.rho; q_new[o + P.N] = q.u; q_new[o + 2 * P.N] = q.v; q_new[o + 3 * P.N] = q.w; q_new[o + 4 * P.N] = q.T; q_new[o + 5 * P.N] = q.mu; q_new[o + 6 * P.N] = q.H;
+        q_new[o] = q.rho; q_new[o + P.QS] = q.u; q_new[o + 2 * P.QS] = q.v; q_new[o + 3 * P.QS] = q.w; q_new[o + 4 * P.QS] = q.T; q_new[o + 5 * P.QS] = q.mu; q_new[o + 6 * P.QS] = q.H;
       }
     }
   }

@@ -51,7 +51,11 @@ struct streams_ctx {
   dim3 rhs_grid;
   int lz;
   size_t istride;                      // entries per direction of ilist
-  int dt_ready;                        // sc->dt_next holds the CFL step of the current state (last k_force_fix of a step)
+  int dt_ready;                        // sc->red[2] holds the CFL maximum of the current state (last k_force_fix of a step)
+  int zpad;                            // ghost planes stored around each state buffer (3 with a BC_HALO z face)
+  int stage_next;                      // staged stepping: -1 = between steps, else the stage whose streams_stage_rhs /
+  int stage_half;                      // streams_stage_end comes next (half: 0 = rhs pending, 1 = end pending)
+  int parts_done;                      // bit 0: interior chunks launched, bit 1: boundary chunks launched (this stage)
   CUtensorMap tmap[2];           // TMA descriptors of qbuf[0], qbuf[1] as 4-D tensors (x, y, z, field)
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
   int prof_on, prof_n;
@@ -129,7 +133,8 @@ const char* validate(const streams_grid* g, const streams_params* p) {
     if (lo == STREAMS_BC_PERIODIC && !(g->len[d] > 0.0)) return "periodic directions need len > 0";
     for (int s = 0; s < 2; ++s) {
       const int b = p->bc[2 * d + s];
-      if (b < 0 || b > STREAMS_BC_WALL_ISO_CHAR) return "unknown boundary kind";
+      if (b < 0 || b > STREAMS_BC_HALO) return "unknown boundary kind";
+      if (b == STREAMS_BC_HALO && d != 2) return "HALO (z-slab decomposition) is supported on z faces only";
       if (b == STREAMS_BC_WALL_ISO_CHAR && !(d == 1 && s == 0)) return "WALL_ISO_CHAR is supported on ymin only";
       if ((b == STREAMS_BC_WALL_ISO_STAGGERED || b == STREAMS_BC_WALL_ISO_NODE) && d != 1) return "walls are supported on y faces only";
       if (b == STREAMS_BC_INFLOW_FROZEN && !(d == 0 && s == 0)) return "INFLOW_FROZEN is supported on xmin only";
@@ -138,6 +143,10 @@ const char* validate(const streams_grid* g, const streams_params* p) {
     }
   }
   if (p->forcing && p->bc[0] != STREAMS_BC_PERIODIC) return "bulk forcing needs a periodic x direction";
+  if (p->bc[4] == STREAMS_BC_HALO || p->bc[5] == STREAMS_BC_HALO) {
+    if (p->weno_enable && p->forcing) return "z-slabs: forcing and the hybrid switch together are not supported";
+    if (p->bc[0] == STREAMS_BC_INFLOW_FROZEN) return "z-slabs: INFLOW_FROZEN is not supported (the frozen plane has no ghost planes)";
+  }
   return nullptr;
 }
 
@@ -203,13 +212,16 @@ bool make_tile_map(CUtensorMap* tm, double* q, int nx, int ny, int nz) {
 
 struct Carve { size_t off = 0; size_t take(size_t bytes) { size_t o = off; off += up(bytes); return o; } };
 
-struct Layout { size_t w[2], S[2], theta, nflag, fbits, lmask, list, ilist, dFbuf, dFb, partial, inflow, speeds, total; int npartial; dim3 grid; int lz; size_t istride; };
+struct Layout { size_t w[2], S[2], theta, nflag, fbits, lmask, list, ilist, dFbuf, dFb, partial, inflow, speeds, sc, total; int npartial; dim3 grid; int lz; size_t istride; int zpad; };
 
 Layout make_layout(const streams_grid& g, const streams_params& p) {
   Layout L;
   const size_t N = (size_t)g.nx * g.ny * g.nz;
   Carve c;
-  for (int i = 0; i < 2; ++i) L.w[i] = c.take(NQ * N * sizeof(double));
+  // a BC_HALO z face stores three ghost planes below AND above each state buffer (the neighbouring slab's planes)
+  L.zpad = (p.bc[4] == STREAMS_BC_HALO || p.bc[5] == STREAMS_BC_HALO) ? HALO : 0;
+  const size_t NS = (size_t)g.nx * g.ny * (g.nz + 2 * L.zpad);
+  for (int i = 0; i < 2; ++i) L.w[i] = c.take(NQ * NS * sizeof(double));
   for (int i = 0; i < 2; ++i) L.S[i] = c.take(5 * N * sizeof(double));
   L.theta = L.nflag = L.fbits = L.lmask = L.list = L.ilist = L.dFbuf = L.dFb = 0;
   if (p.weno_enable) {
@@ -245,6 +257,9 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
       if (lz == 1) break;
     }
   }
+  // z-slabs: at least four chunks where the slab allows it, so that the chunks between the two boundary chunks (which
+  // need no ghost plane) can run while the halo exchange is in flight (Fig. 8)
+  if (L.zpad) nchunk = std::max(nchunk, std::min(4, std::max(1, g.nz / 8)));
   L.lz = (g.nz + nchunk - 1) / nchunk;
   nchunk = (g.nz + L.lz - 1) / L.lz;
   L.grid = dim3(tiles_x, tiles_y, nchunk);
@@ -252,6 +267,7 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   L.partial = c.take((size_t)L.npartial * sizeof(double));
   L.inflow = c.take((size_t)NQ * g.nz * g.ny * sizeof(double));
   L.speeds = c.take(8 * sizeof(double));
+  L.sc = c.take(sizeof(DevScal));        // device scalars in caller memory: the caller may run collectives on streams_reduce_ptr
   L.total = c.off;
   return L;
 }
@@ -360,7 +376,9 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   // stream capture is not allowed on the legacy default stream: graphs need a stream of the caller's own
   c->graph_ok = (c->st != nullptr && c->st != cudaStreamLegacy && c->st != cudaStreamPerThread) ? 1 : 0;
   char* base = (char*)d_workspace;
-  for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]); c->S[i] = (double*)(base + L.S[i]); }
+  c->zpad = L.zpad;
+  const size_t zoff = (size_t)L.zpad * g->nx * g->ny;      // qbuf points at the first INTERIOR plane
+  for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]) + zoff; c->S[i] = (double*)(base + L.S[i]); }
   if (p->weno_enable) {
     c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
     c->fbits = (unsigned int*)(base + L.fbits); c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
@@ -368,10 +386,16 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   }
   c->partial = (double*)(base + L.partial); c->inflow = (double*)(base + L.inflow); c->speeds = (double*)(base + L.speeds);
   c->npartial = L.npartial; c->rhs_grid = L.grid; c->lz = L.lz; c->istride = L.istride;
+  c->sc = (DevScal*)(base + L.sc);
+  c->stage_next = -1;
 
   // ---- S1 ghost coordinates and S2 metrics (host, O(n)) ----
   const int n[3] = {g->nx, g->ny, g->nz};
-  const double* xin[3] = {hx, hy, hz};
+  // h_z of a slab: [3 ghost coordinates if bc[zmin] == HALO][nz nodes][3 ghost coordinates if bc[zmax] == HALO]
+  const double* hz_lo = p->bc[4] == STREAMS_BC_HALO ? hz : nullptr;
+  const double* hz_in = hz + (hz_lo ? HALO : 0);
+  const double* hz_hi = p->bc[5] == STREAMS_BC_HALO ? hz_in + g->nz : nullptr;
+  const double* xin[3] = {hx, hy, hz_in};
   Coef K;
   coeffs(p->order, K);
   std::vector<double> ih[3], gh[3], hh[3], xg0;
@@ -386,7 +410,10 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
         const int gi = s == 0 ? -l : n[d] - 1 + l;
         const int bc = p->bc[2 * d + s];
         double v;
-        if (bc == STREAMS_BC_PERIODIC) {
+        if (bc == STREAMS_BC_HALO) {
+          v = s == 0 ? hz_lo[HALO - l] : hz_hi[l - 1];       // the neighbouring slab's node coordinates
+          if (s == 0 ? !(v < xin[d][0]) : !(v > xin[d][n[d] - 1])) { delete c; return fail(nullptr, STREAMS_EINVAL, "HALO ghost coordinates must continue the z nodes monotonically"); }
+        } else if (bc == STREAMS_BC_PERIODIC) {
           int r = gi % n[d]; if (r < 0) r += n[d];
           v = xin[d][r] + (double)((gi - r) / n[d]) * g->len[d];
         } else if (bc == STREAMS_BC_WALL_ISO_STAGGERED) {
@@ -419,6 +446,7 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   // ---- device parameter block ----
   DevP& P = c->P;
   P.nx = n[0]; P.ny = n[1]; P.nz = n[2]; P.nxy = n[0] * n[1]; P.N = (long long)n[0] * n[1] * n[2];
+  P.zpad = L.zpad; P.QS = (long long)n[0] * n[1] * (n[2] + 2 * L.zpad);
   for (int i = 0; i < 6; ++i) P.bc[i] = p->bc[i];
   P.visc_model = p->visc_model; P.weno = p->weno_enable; P.forcing = p->forcing; P.viscous = p->viscous_enable; P.L = p->order / 2;
   P.gam = p->gamma; P.gm1 = p->gamma - 1.0; P.Rgas = p->Rgas; P.inv_R = 1.0 / p->Rgas;
@@ -441,10 +469,9 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   }
 
   // ---- small device arrays ----
-  size_t off = 0, o_arr[9], o_xpost, o_sc, o_stat;
+  size_t off = 0, o_arr[9], o_xpost, o_stat;
   for (int a = 0; a < 9; ++a) { o_arr[a] = off; off += up((size_t)n[a % 3] * sizeof(double)); }
   o_xpost = off; off += up(xpost.size());
-  o_sc = off; off += up(sizeof(DevScal));
   o_stat = off; off += up(((size_t)(STAT_ZC + 1) * NSTAT * n[1] + 1) * sizeof(double));
   cudaError_t e = cudaMalloc(&c->small_dev, off);
   if (e != cudaSuccess) { delete c; return cuda_fail(nullptr, e, "cudaMalloc(metrics)"); }
@@ -458,7 +485,6 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   cudaMemcpyAsync(sb + o_xpost, xpost.data(), xpost.size(), cudaMemcpyHostToDevice, c->st);
   P.xpost = (const unsigned char*)(sb + o_xpost);
   P.inflow = c->inflow;
-  c->sc = (DevScal*)(sb + o_sc);
   c->stat_partial = (double*)(sb + o_stat);
   c->stat_sum = c->stat_partial + (size_t)STAT_ZC * NSTAT * n[1];
   c->stat_n = (unsigned long long*)(c->stat_sum + (size_t)NSTAT * n[1]);
@@ -475,7 +501,7 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   c->use_tma = (n[0] % 2 == 0) ? 1 : 0;
   if (c->use_tma)
     for (int i = 0; i < 2; ++i)
-      if (!make_tile_map(&c->tmap[i], c->qbuf[i], n[0], n[1], n[2])) {
+      if (!make_tile_map(&c->tmap[i], c->qbuf[i] - zoff, n[0], n[1], n[2] + 2 * L.zpad)) {
         cudaFree(c->small_dev); delete c;
         return fail(nullptr, STREAMS_ECUDA, "cuTensorMapEncodeTiled failed");
       }
@@ -503,7 +529,7 @@ static int after_set_state(streams_ctx* c, const double* d_w) {
   CK(cudaMemsetAsync(&c->sc->force, 0, sizeof(double), c->st));
   CK(cudaMemsetAsync(&c->sc->time, 0, sizeof(double), c->st));
   if (!(c->p.dt_fixed > 0.0)) CK(cudaMemsetAsync(&c->sc->dt, 0, sizeof(double), c->st));
-  c->has_state = 1; c->step = 0; c->scur = 0; c->dt_ready = 0;
+  c->has_state = 1; c->step = 0; c->scur = 0; c->dt_ready = 0; c->stage_next = -1; c->stage_half = 0; c->parts_done = 0;
   return STREAMS_OK;
 }
 
@@ -589,7 +615,7 @@ static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, d
   return STREAMS_OK;
 }
 
-static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in) {
+static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in, dim3 grid) {
   RhsArgs A = A_in;
   A.use_tma = c->use_tma;
   A.nflag = c->p.weno_enable ? c->nflag : nullptr;
@@ -597,22 +623,22 @@ static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in) {
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
-  if (mode == 2) k_rhs<2><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);       // fused RK stage, lazy forcing
-  else if (mode == 1) k_rhs<1><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);  // fused RK stage
-  else k_rhs<0><<<c->rhs_grid, NT, smem, c->st>>>(c->P, A, tm);                 // residual only
+  if (mode == 2) k_rhs<2><<<grid, NT, smem, c->st>>>(c->P, A, tm);       // fused RK stage, lazy forcing
+  else if (mode == 1) k_rhs<1><<<grid, NT, smem, c->st>>>(c->P, A, tm);  // fused RK stage
+  else k_rhs<0><<<grid, NT, smem, c->st>>>(c->P, A, tm);                 // residual only
   LAUNCH_CHECK("k_rhs");
   if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
 }
 
-static int force_from_partials(streams_ctx* c, const double* R, bool have_rhs_partials) {
+static int force_from_partials(streams_ctx* c, const double* R, bool have_rhs_partials, bool take) {
   int n = (int)(c->rhs_grid.x * c->rhs_grid.y * c->rhs_grid.z);
   if (!have_rhs_partials) {
     n = rgrid_for(c->P.N);
     k_force_partial<<<n, RT, 0, c->st>>>(c->P, R, c->partial);
     LAUNCH_CHECK("k_force_partial");
   }
-  k_force_final<<<1, RT, 0, c->st>>>(c->partial, n, c->sc);
+  k_force_final<<<1, RT, 0, c->st>>>(c->partial, n, c->sc, take ? 1 : 0);
   LAUNCH_CHECK("k_force_final");
   return STREAMS_OK;
 }
@@ -625,15 +651,15 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   int rc;
   RhsArgs A;
   std::memset(&A, 0, sizeof A);
-  A.q = w; A.out_rhs = d_rhs; A.lz = c->lz;
+  A.q = w; A.out_rhs = d_rhs; A.lz = c->lz; A.cz0 = 0; A.czs = 1;
   const bool partial_ok = c->p.forcing && !c->p.weno_enable;
   A.partial = partial_ok ? c->partial : nullptr;
-  if ((rc = launch_rhs(c, 0, A))) return rc;
+  if ((rc = launch_rhs(c, 0, A, c->rhs_grid))) return rc;
   if (c->p.weno_enable) {
     if ((rc = run_weno(c, w, d_rhs, nullptr, 0.0))) return rc;
   }
   if (c->p.forcing) {
-    if ((rc = force_from_partials(c, d_rhs, partial_ok))) return rc;
+    if ((rc = force_from_partials(c, d_rhs, partial_ok, true))) return rc;
     k_apply_force<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, w, d_rhs, c->sc);
     LAUNCH_CHECK("k_apply_force");
   }
@@ -651,72 +677,114 @@ int streams_sensor(streams_ctx* c, double* d_theta, unsigned char* d_flags) {
 // host state that decides which kernels one RK3 step launches and on which buffers
 static int step_key(const streams_ctx* c) { return c->cur | (c->scur << 1) | (c->dt_ready << 2); }
 
-// enqueue ONE RK3 step (Eq. 11) on the context stream and advance the host-side state (buffers, dt_ready)
-static int step_once(streams_ctx* c) {
-  static const double alpha[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};   // Eq. 11 with the sign of reading G5
-  static const double beta[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
+static const double RK_ALPHA[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};   // Eq. 11 with the sign of reading G5
+static const double RK_BETA[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
+enum { PART_ALL = 0, PART_INTERIOR = 1, PART_BOUNDARY = 2 };
+
+// S10, first half: the CFL maximum of the current state into sc->red[2] (already there after a lazy-forcing step)
+static int do_step_begin(streams_ctx* c) {
+  if (c->p.dt_fixed > 0.0 || c->dt_ready) return STREAMS_OK;
   const int rg = rgrid_for(c->P.N);
+  k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->partial);
+  LAUNCH_CHECK("k_speed_partial");
+  k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->sc, nullptr, 1);
+  LAUNCH_CHECK("k_dt_final");
+  return STREAMS_OK;
+}
+
+// chunks of the fused kernel launched by one part: whole grid, the chunks between the first and the last one (they read
+// no ghost plane of a z face), or the first and the last chunk
+static bool part_chunks(const streams_ctx* c, int part, RhsArgs& A, dim3& grid) {
+  const int nch = (int)c->rhs_grid.z;
+  grid = c->rhs_grid;
+  A.cz0 = 0; A.czs = 1;
+  if (part == PART_INTERIOR) { if (nch < 3) return false; A.cz0 = 1; grid.z = nch - 2; }
+  if (part == PART_BOUNDARY) { A.czs = std::max(1, nch - 1); grid.z = std::min(2, nch); }
+  return true;
+}
+
+// first half of RK stage l (Eq. 11): dt (l = 0), the fused residual + stage kernel, and the partial body-force sums
+// into sc->red[0..1].  part: PART_ALL, or PART_INTERIOR then PART_BOUNDARY (the reductions follow the boundary part).
+static int do_stage_rhs(streams_ctx* c, int l, int part, bool single) {
   int rc;
-  if (!(c->p.dt_fixed > 0.0) && c->dt_ready) {
-    k_take_dt<<<1, 1, 0, c->st>>>(c->sc);
+  const bool first = part != PART_BOUNDARY, last = part != PART_INTERIOR;
+  if (l == 0 && first && !(c->p.dt_fixed > 0.0)) {
+    k_take_dt<<<1, 1, 0, c->st>>>(c->sc, c->p.cfl);
     LAUNCH_CHECK("k_take_dt");
     c->dt_ready = 0;
-  } else if (!(c->p.dt_fixed > 0.0)) {
-    k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, c->qbuf[c->cur], c->partial);
-    LAUNCH_CHECK("k_speed_partial");
-    k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 1);
-    LAUNCH_CHECK("k_dt_final");
   }
-  for (int l = 0; l < 3; ++l) {
-    double* w = c->qbuf[c->cur];
-    RhsArgs A;
-    std::memset(&A, 0, sizeof A);
-    A.q = w; A.lz = c->lz; A.alpha = alpha[l]; A.beta = beta[l]; A.dt_ptr = &c->sc->dt;
-    if (c->p.forcing && !c->p.weno_enable) {
-      // lazy forcing: the fused kernel advances with alpha (R_prev + f_prev ...) + beta R and sums R_rhou; once f is
-      // known a light kernel adds dt beta f (e_rhou + u e_rhoE).  S[0] keeps R without the forcing terms.
-      double* wn = c->qbuf[c->cur ^ 1];
-      A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
-      A.f_prev = l > 0 ? &c->sc->force : nullptr;
-      A.write_S = l < 2 ? 1 : 0;
-      if ((rc = launch_rhs(c, 2, A))) return rc;
-      if ((rc = force_from_partials(c, nullptr, true))) return rc;
-      const bool want_dt = l == 2 && !(c->p.dt_fixed > 0.0);
-      k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, beta[l], want_dt ? c->partial : nullptr);
-      LAUNCH_CHECK("k_force_fix");
-      if (want_dt) {
-        k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, nullptr, 2);
-        LAUNCH_CHECK("k_dt_final");
-        c->dt_ready = 1;
-      }
-      c->cur ^= 1;
-    } else if (c->p.forcing) {
-      // R -> S[scur^1]; f from the reduction; then the update kernel (Eq. 11 + S9)
-      double* Sp = c->S[c->scur];
-      double* Sc = c->S[c->scur ^ 1];
-      const bool partial_ok = !c->p.weno_enable;
-      A.out_rhs = Sc; A.partial = partial_ok ? c->partial : nullptr;
-      if ((rc = launch_rhs(c, 0, A))) return rc;
-      if (c->p.weno_enable) {
-        if ((rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
-      }
-      if ((rc = force_from_partials(c, Sc, partial_ok))) return rc;
-      k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, alpha[l], beta[l], 1, l < 2 ? 1 : 0);
-      LAUNCH_CHECK("k_update");
-      c->scur ^= 1;
-    } else {
-      // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
-      double* wn = c->qbuf[c->cur ^ 1];
-      A.q_out = wn; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
-      if ((rc = launch_rhs(c, 1, A))) return rc;
-      if (c->p.weno_enable) {
-        if ((rc = run_weno(c, w, c->S[0], wn, beta[l]))) return rc;
-      }
-      c->cur ^= 1;
+  double* w = c->qbuf[c->cur];
+  RhsArgs A;
+  std::memset(&A, 0, sizeof A);
+  A.q = w; A.lz = c->lz; A.alpha = RK_ALPHA[l]; A.beta = RK_BETA[l]; A.dt_ptr = &c->sc->dt;
+  dim3 grid;
+  const bool any = part_chunks(c, part, A, grid);
+  if (c->p.forcing && !c->p.weno_enable) {
+    // lazy forcing: the fused kernel advances with alpha (R_prev + f_prev ...) + beta R and sums R_rhou; once f is
+    // known a light kernel adds dt beta f (e_rhou + u e_rhoE).  S[0] keeps R without the forcing terms.
+    A.q_out = c->qbuf[c->cur ^ 1]; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.partial = c->partial;
+    A.f_prev = l > 0 ? &c->sc->force : nullptr;
+    A.write_S = l < 2 ? 1 : 0;
+    if (any && (rc = launch_rhs(c, 2, A, grid))) return rc;
+    if (last && (rc = force_from_partials(c, nullptr, true, single))) return rc;
+  } else if (c->p.forcing) {
+    // forcing with the hybrid switch: R -> S[scur^1]; WENO, f and the update kernel follow in do_stage_end
+    const bool partial_ok = !c->p.weno_enable;
+    A.out_rhs = c->S[c->scur ^ 1]; A.partial = partial_ok ? c->partial : nullptr;
+    if (any && (rc = launch_rhs(c, 0, A, grid))) return rc;
+  } else {
+    // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
+    A.q_out = c->qbuf[c->cur ^ 1]; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
+    if (any && (rc = launch_rhs(c, 1, A, grid))) return rc;
+  }
+  return STREAMS_OK;
+}
+
+// second half of RK stage l: f = -red[0] / red[1] (combined across z-slabs by the caller), the forcing fix, the WENO
+// correction; after the last stage the CFL maximum of the new state and the time
+static int do_stage_end(streams_ctx* c, int l, bool single) {
+  const int rg = rgrid_for(c->P.N);
+  int rc;
+  double* w = c->qbuf[c->cur];
+  if (c->p.forcing && !c->p.weno_enable) {
+    double* wn = c->qbuf[c->cur ^ 1];
+    if (!single) { k_force_take<<<1, 1, 0, c->st>>>(c->sc); LAUNCH_CHECK("k_force_take"); }
+    const bool want_dt = l == 2 && !(c->p.dt_fixed > 0.0);
+    k_force_fix<<<rg, RT, 0, c->st>>>(c->P, wn, w, c->sc, RK_BETA[l], want_dt ? c->partial : nullptr);
+    LAUNCH_CHECK("k_force_fix");
+    if (want_dt) {
+      k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->sc, nullptr, 1);
+      LAUNCH_CHECK("k_dt_final");
+      c->dt_ready = 1;
     }
+    c->cur ^= 1;
+  } else if (c->p.forcing) {
+    double* Sp = c->S[c->scur];
+    double* Sc = c->S[c->scur ^ 1];
+    if (c->p.weno_enable && (rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
+    if ((rc = force_from_partials(c, Sc, !c->p.weno_enable, true))) return rc;
+    k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, RK_ALPHA[l], RK_BETA[l], 1, l < 2 ? 1 : 0);
+    LAUNCH_CHECK("k_update");
+    c->scur ^= 1;
+  } else {
+    if (c->p.weno_enable && (rc = run_weno(c, w, c->S[0], c->qbuf[c->cur ^ 1], RK_BETA[l]))) return rc;
+    c->cur ^= 1;
   }
-  k_advance_time<<<1, 1, 0, c->st>>>(c->sc);
-  LAUNCH_CHECK("k_advance_time");
+  if (l == 2) {
+    k_advance_time<<<1, 1, 0, c->st>>>(c->sc);
+    LAUNCH_CHECK("k_advance_time");
+  }
+  return STREAMS_OK;
+}
+
+// enqueue ONE RK3 step (Eq. 11) on the context stream and advance the host-side state (buffers, dt_ready)
+static int step_once(streams_ctx* c) {
+  int rc;
+  if ((rc = do_step_begin(c))) return rc;
+  for (int l = 0; l < 3; ++l) {
+    if ((rc = do_stage_rhs(c, l, PART_ALL, true))) return rc;
+    if ((rc = do_stage_end(c, l, true))) return rc;
+  }
   return STREAMS_OK;
 }
 
@@ -728,6 +796,8 @@ int streams_step(streams_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return fail(c, STREAMS_EINVAL, "bad argument");
   DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  if (c->zpad) return fail(c, STREAMS_EINVAL, "a z-slab (BC_HALO) advances by the staged calls: its ghost planes are exchanged between stages");
+  if (c->stage_next >= 0) return fail(c, STREAMS_ESTATE, "a staged step is open (streams_step_begin without the third streams_stage_end)");
   int rc;
   for (int s = 0; s < nsteps; ++s) {
     const bool graph = c->graph_ok && !c->prof_on && c->P.N < GRAPH_MAX_POINTS;
@@ -762,6 +832,73 @@ int streams_step(streams_ctx* c, int nsteps) {
     c->step++;
   }
   return STREAMS_OK;
+}
+
+// ---- staged stepping and z-slab halos ----------------------------------------------------
+
+int streams_step_begin(streams_ctx* c) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  if (c->stage_next >= 0) return fail(c, STREAMS_ESTATE, "streams_step_begin: the previous staged step is not finished");
+  const int rc = do_step_begin(c);
+  if (rc) return rc;
+  c->stage_next = 0; c->stage_half = 0; c->parts_done = 0;
+  return STREAMS_OK;
+}
+
+int streams_stage_rhs(streams_ctx* c, int stage, int part) {
+  if (!c || part < PART_ALL || part > PART_BOUNDARY) return fail(c, STREAMS_EINVAL, "bad argument");
+  DevGuard dg(c->device);
+  if (c->stage_next != stage || c->stage_half != 0) return fail(c, STREAMS_ESTATE, "streams_stage_rhs out of order (step_begin, then rhs / end of stages 0, 1, 2)");
+  if (part == PART_ALL && c->parts_done) return fail(c, STREAMS_ESTATE, "streams_stage_rhs: PART_ALL after a partial launch");
+  if (part == PART_INTERIOR && c->parts_done) return fail(c, STREAMS_ESTATE, "streams_stage_rhs: the interior part comes first, once");
+  if (part == PART_BOUNDARY && (c->parts_done & 2)) return fail(c, STREAMS_ESTATE, "streams_stage_rhs: boundary part launched twice");
+  int rc;
+  if (part == PART_BOUNDARY && !(c->parts_done & 1)) {
+    // no interior launch was asked for: the boundary part then stands for the whole grid
+    part = PART_ALL;
+  }
+  if ((rc = do_stage_rhs(c, stage, part, false))) return rc;
+  if (part == PART_INTERIOR) c->parts_done = 1;
+  else { c->parts_done = 3; c->stage_half = 1; }
+  return STREAMS_OK;
+}
+
+int streams_stage_end(streams_ctx* c, int stage) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
+  if (c->stage_next != stage || c->stage_half != 1) return fail(c, STREAMS_ESTATE, "streams_stage_end out of order");
+  const int rc = do_stage_end(c, stage, false);
+  if (rc) return rc;
+  c->stage_half = 0; c->parts_done = 0;
+  if (stage == 2) { c->stage_next = -1; c->step++; } else c->stage_next = stage + 1;
+  return STREAMS_OK;
+}
+
+double* streams_reduce_ptr(streams_ctx* c) { return c ? c->sc->red : nullptr; }
+
+size_t streams_halo_bytes(const streams_ctx* c) { return c ? (size_t)NQ * HALO * c->P.nxy * sizeof(double) : 0; }
+
+// the three planes next to a z face <-> a contiguous message [NQ][3][ny][nx] (seven copies of 3 nx ny doubles)
+static int halo_copy(streams_ctx* c, int face, double* buf, void* stream, bool pack) {
+  if (!c || !buf || (face != 4 && face != 5)) return fail(c, STREAMS_EINVAL, "bad argument (face: 4 = zmin, 5 = zmax)");
+  DevGuard dg(c->device);
+  if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  if (!pack && c->p.bc[face] != STREAMS_BC_HALO) return fail(c, STREAMS_EINVAL, "streams_halo_unpack: this face is not BC_HALO");
+  cudaStream_t st = stream ? (cudaStream_t)stream : c->st;
+  const long long k = pack ? (face == 4 ? 0 : c->P.nz - HALO) : (face == 4 ? -HALO : c->P.nz);
+  const size_t n = (size_t)HALO * c->P.nxy;
+  double* q = c->qbuf[c->cur] + k * c->P.nxy;
+  for (int f = 0; f < NQ; ++f) {
+    if (pack) CK(cudaMemcpyAsync(buf + f * n, q + f * c->P.QS, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    else CK(cudaMemcpyAsync(q + f * c->P.QS, buf + f * n, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  }
+  return STREAMS_OK;
+}
+int streams_halo_pack(streams_ctx* c, int face, double* d_buf, void* cuda_stream) { return halo_copy(c, face, d_buf, cuda_stream, true); }
+int streams_halo_unpack(streams_ctx* c, int face, const double* d_buf, void* cuda_stream) {
+  return halo_copy(c, face, const_cast<double*>(d_buf), cuda_stream, false);
 }
 
 int streams_stats_accumulate(streams_ctx* c) {
@@ -812,7 +949,7 @@ int streams_diagnostics(streams_ctx* c, streams_diag* out) {
   CK(cudaMemcpyAsync(c->h_sc, c->sc, sizeof hs, cudaMemcpyDeviceToHost, c->st));
   k_speed_partial<<<rg, RT, 0, c->st>>>(c->P, w, c->partial);
   LAUNCH_CHECK("k_speed_partial");
-  k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->p.cfl, c->p.dt_fixed, c->sc, c->speeds, 0);
+  k_dt_final<<<1, RT, 0, c->st>>>(c->partial, rg, c->sc, c->speeds, 0);
   LAUNCH_CHECK("k_dt_final");
   double* sp = c->h_part + (size_t)NDIAG * RGRID;
   CK(cudaMemcpyAsync(sp, c->speeds, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->st));

@@ -1,0 +1,245 @@
+"""z-slab decomposition on ONE GPU: several contexts of the CUDA library,
+one per slab, exchange their ghost planes through the C-ABI halo calls and are stepped by the staged calls.
+
+What the decomposed run must compute is fixed by the undivided problem: it is compared (a) bit for bit with the
+single-context run of the same library (every node sees the same stencil values; the maximum of S10 is exact; the body-force
+sum of S9 is either fed from the undivided run -> bitwise, or combined from the slabs' partial sums -> summation-order
+round-off only) and (b) with the CPU oracle on the undivided grid, to the step tolerance of DESIGN.md A18.
+Kernels of different slabs never wait on one another: the exchange is ordered by stream events on one device.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+STEP_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2004_02276_b200 import build
+    build.build()
+    from paper_2004_02276_b200 import binding, slab
+    from oracle import binding as ob
+    binding.lib()
+    return torch, binding, slab, ob
+
+
+class HostReducer:
+    """Combines the slabs' partial reductions on the host (test only): fixed slab order."""
+
+    def __init__(self, torch):
+        self.torch = torch
+
+    def _combine(self, slabs, lo, hi, fn):
+        vals = []
+        for s in slabs:
+            s.stream.synchronize()
+            vals.append(s.red[lo:hi].cpu().numpy().copy())
+        tot = vals[0]
+        for v in vals[1:]:
+            tot = fn(tot, v)
+        t = self.torch.from_numpy(tot)
+        for s in slabs:
+            with self.torch.cuda.stream(s.stream):
+                s.red[lo:hi].copy_(t.to(s.device))
+            s.stream.synchronize()
+
+    def sum(self, slabs, syncs):
+        self._combine(slabs, 0, 2, lambda a, b: a + b)
+
+    def max(self, slabs, syncs):
+        self._combine(slabs, 2, 3, np.maximum)
+
+
+def make_slabs(env, wl, nslabs):
+    torch, binding, slab, _ = env
+    w0 = wl.state()
+    ctxs, specs = [], []
+    for r in range(nslabs):
+        sp = slab.slab_spec(wl.grid, wl.z, wl.params, nslabs, r)
+        c = binding.Streams(sp.grid, wl.x, wl.y, sp.z, sp.params)
+        c.set_state(torch.from_numpy(np.ascontiguousarray(w0[:, sp.k0:sp.k1])).cuda())
+        ctxs.append(c)
+        specs.append(sp)
+    return ctxs, specs, w0
+
+
+def gather(ctxs):
+    return np.concatenate([c.get_state().cpu().numpy() for c in ctxs], axis=1)
+
+
+def l2(a, b):
+    return max(np.linalg.norm(a[v] - b[v]) / np.linalg.norm(b[v]) for v in range(5))
+
+
+@pytest.mark.parametrize("nslabs,overlap", [(2, False), (3, True), (4, True)])
+def test_periodic_box_slabs_are_bitwise_the_undivided_run(env, nslabs, overlap):
+    """No forcing, CFL time step (max-reduction across slabs): the concatenated slabs equal the single context bit for bit,
+    with and without the interior / boundary split of the fused kernel."""
+    torch, binding, slab, ob = env
+    wl = W.random_periodic(40, 20, 48, params=W.default_params(Rgas=1 / 1.4, mu_ref=5e-3))
+    w0 = wl.state()
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(w0).cuda())
+    one.step(3)
+    ref = one.get_state().cpu().numpy()
+    ctxs, specs, _ = make_slabs(env, wl, nslabs)
+    grp = slab.SlabGroup(ctxs, nslabs, periodic=True, reducer=HostReducer(torch), forcing=False, cfl_dt=True, overlap=overlap)
+    grp.step(3)
+    got = gather(ctxs)
+    assert np.array_equal(got, ref), np.abs(got - ref).max()
+    assert grp.messages_sent == 3 * 3 * 2 * nslabs
+    d1, ds = one.diagnostics(), [c.diagnostics() for c in ctxs]
+    assert all(d.dt == d1.dt and d.time == d1.time and d.step == 3 for d in ds)
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    o.set_state(w0)
+    o.step(3)
+    assert l2(got, o.get_state()) < STEP_TOL
+    for c in ctxs + [one]:
+        c.close()
+    o.close()
+
+
+def test_slab_residual_equals_the_undivided_residual(env):
+    """streams_rhs on slabs after one halo swap = the rows of the undivided residual, bit for bit."""
+    torch, binding, slab, ob = env
+    wl = W.random_periodic(36, 18, 30, params=W.default_params(Rgas=1 / 1.4, mu_ref=5e-3), stretched_y=True)
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(wl.state()).cuda())
+    ref = one.rhs().cpu().numpy()
+    ctxs, specs, _ = make_slabs(env, wl, 3)
+    grp = slab.SlabGroup(ctxs, 3, periodic=True, reducer=HostReducer(torch))
+    grp.residual_ready()
+    got = np.concatenate([c.rhs().cpu().numpy() for c in ctxs], axis=1)
+    assert np.array_equal(got, ref), np.abs(got - ref).max()
+    for c in ctxs + [one]:
+        c.close()
+
+
+def test_channel_slabs_with_forcing(env):
+    """Lazy forcing across slabs: the body force needs the sum of R_rhou vol over ALL slabs every stage.
+    (1) fed: the staged calls on the undivided context run in lockstep and its red[] goes to every slab -> bitwise;
+    (2) combined: the slabs' partial sums are added (another summation order) -> round-off; oracle parity for both."""
+    torch, binding, slab, ob = env
+    wl = W.config3_channel(64, 32, 40)
+    w0 = wl.state()
+    nsl, nsteps = 2, 3
+    # (1) fed
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(w0).cuda())
+    ctxs, specs, _ = make_slabs(env, wl, nsl)
+    grp = slab.SlabGroup(ctxs, nsl, periodic=True, reducer=HostReducer(torch), forcing=True)
+
+    def feed(lo, hi):
+        one.stream.synchronize()
+        v = one.red[lo:hi].clone()
+        for c in ctxs:
+            with torch.cuda.stream(c.stream):
+                c.red[lo:hi].copy_(v)
+            c.stream.synchronize()
+
+    for _ in range(nsteps):
+        one.step_begin()
+        for c in ctxs:
+            c.step_begin()
+        feed(2, 3)
+        for stage in range(3):
+            ready = grp.swap_halos()
+            one.stage_rhs(stage, one.PART_ALL)
+            for i, c in enumerate(ctxs):
+                grp.syncs[i].main_wait(ready[i])
+                c.stage_rhs(stage, c.PART_INTERIOR)
+                c.stage_rhs(stage, c.PART_BOUNDARY)
+            feed(0, 2)
+            one.stage_end(stage)
+            for c in ctxs:
+                c.stage_end(stage)
+    ref = one.get_state().cpu().numpy()
+    got = gather(ctxs)
+    assert np.array_equal(got, ref), np.abs(got - ref).max()
+    # the staged calls on one context are streams_step
+    two = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    two.set_state(torch.from_numpy(w0).cuda())
+    two.step(nsteps)
+    assert np.array_equal(two.get_state().cpu().numpy(), ref)
+    # (2) combined
+    ctxs2, _, _ = make_slabs(env, wl, nsl)
+    grp2 = slab.SlabGroup(ctxs2, nsl, periodic=True, reducer=HostReducer(torch), forcing=True)
+    grp2.step(nsteps)
+    got2 = gather(ctxs2)
+    assert l2(got2, ref) < 1e-13
+    f1, f2 = one.diagnostics().forcing, ctxs2[0].diagnostics().forcing
+    assert abs(f1 - f2) <= 1e-12 * abs(f1)
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    o.set_state(w0)
+    o.step(nsteps)
+    assert l2(got2, o.get_state()) < STEP_TOL
+    for c in ctxs + ctxs2 + [one, two]:
+        c.close()
+    o.close()
+
+
+def test_staged_calls_enforce_their_order(env):
+    torch, binding, slab, _ = env
+    wl = W.random_periodic(32, 16, 16, params=W.default_params(Rgas=1 / 1.4, mu_ref=5e-3))
+    sp = slab.slab_spec(wl.grid, wl.z, wl.params, 2, 0)
+    c = binding.Streams(sp.grid, wl.x, wl.y, sp.z, sp.params)
+    c.set_state(torch.from_numpy(np.ascontiguousarray(wl.state()[:, sp.k0:sp.k1])).cuda())
+    with pytest.raises(binding.StreamsError):
+        c.step(1)                                    # a slab advances by the staged calls only
+    with pytest.raises(binding.StreamsError):
+        c.stage_rhs(0)                               # before step_begin
+    c.step_begin()
+    with pytest.raises(binding.StreamsError):
+        c.stage_end(0)                               # before stage_rhs
+    with pytest.raises(binding.StreamsError):
+        c.stage_rhs(1)                               # wrong stage
+    c.close()
+    # a non-periodic direction cannot take BC_HALO outside z
+    p = dict(wl.params)
+    p["bc"] = [8, 8, 0, 0, 0, 0]
+    with pytest.raises(binding.StreamsError):
+        binding.Streams(wl.grid, wl.x, wl.y, wl.z, p)
+
+
+def test_nccl_self_exchange_world_size_one(env):
+    """The torch.distributed (NCCL) path of SlabGroup on one GPU: a single periodic slab whose two faces are BC_HALO
+    sends its messages to itself through ncclSend/ncclRecv and all-reduces its partial reductions (world size 1: no rank
+    waits on another rank's kernels).  Result: bitwise the periodic single-context run."""
+    torch, binding, slab, ob = env
+    import torch.distributed as dist
+    if not dist.is_nccl_available():
+        pytest.skip("NCCL backend not available")
+    wl = W.config3_channel(48, 24, 24)
+    w0 = wl.state()
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(w0).cuda())
+    one.step(2)
+    ref = one.get_state().cpu().numpy()
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29533")
+    created = not dist.is_initialized()
+    if created:
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        # one slab of the whole domain, but with both z faces as internal (HALO) boundaries: its own planes come back
+        sp = slab.slab_spec(wl.grid, wl.z, wl.params, 1, 0)
+        assert sp.params["bc"][4] == 8 and sp.params["bc"][5] == 8 and len(sp.z) == wl.grid["nz"] + 6
+        c = binding.Streams(sp.grid, wl.x, wl.y, sp.z, sp.params)
+        c.set_state(torch.from_numpy(w0).cuda())
+        grp = slab.SlabGroup([c], 1, rank=0, periodic=True, dist=dist, forcing=True)
+        grp.step(2)
+        got = c.get_state().cpu().numpy()
+        assert np.array_equal(got, ref), np.abs(got - ref).max()
+        assert grp.messages_sent == 2 * 3 * 2
+        c.close()
+    finally:
+        if created:
+            dist.destroy_process_group()
+    one.close()
