@@ -8,8 +8,11 @@ reductions) of the whole grid through the C-ABI library.  The default workload i
 BASELINE.json configs[4]: the 1024x512x512 supersonic channel block (268M points), the
 configuration the metric is quoted on; it fits one B200 (43 GB workspace).
 
-N > 1: the path does not shard (north_star: one GPU, no decomposition) -> N independent
-replicas, one per rank/GPU, no data-path collective ("replicas only", scaling = weak).
+N = 1 is the metric's configuration (north_star: one GPU, no decomposition, no collectives).
+N > 1 (--decomp auto): the paper's own multi-GPU mode, SURVEY.md 8.f rank 1 -- the channel is N times as long in z, one
+z-slab of the config's size per rank/GPU (weak scaling), ghost planes swapped every RK stage by NCCL send/recv overlapped
+with the slab's interior chunks, two scalar all-reduces per stage/step.  --decomp replicas runs N
+independent copies instead (no data-path collective); --decomp slab at N = 1 is the staged path exchanging with itself.
 
 --impl reference: times the CPU oracle (oracle/, plain C, as it stands) on a bounded slab
 of the same workload on the host cores; rank 0 only.
@@ -34,11 +37,13 @@ UNIT = "points/s"
 PAPER_CONTEXT = "paper: 1 Tesla P100 ~ 330 Intel KNL cores (PAPER.md:11); no absolute throughput published"
 
 
-def make_workload(cfg: int, scale: float = 1.0):
+def make_workload(cfg: int, zcopies: int = 1):
     if cfg == 5:
-        return W.config5_channel_big()
+        return W.config5_channel_big(zcopies=zcopies)
     if cfg == 3:
-        return W.config3_channel()
+        return W.config3_channel(zcopies=zcopies)
+    if zcopies != 1:
+        raise SystemExit("--decomp slab: configs 3 and 5 (channel, periodic z, central scheme) only")
     if cfg == 1:
         return W.config1_tgv()
     if cfg == 2:
@@ -167,13 +172,13 @@ def run_reference(args, rank):
     print(json.dumps(out), flush=True)
 
 
-def upload_state(torch, wl, dev, planes=16):
-    """Generate the seeded initial state slab by slab on the host and place it in HBM."""
-    w = torch.empty(wl.shape, dtype=torch.float64, device=dev)
-    nz = wl.grid["nz"]
-    for k0 in range(0, nz, planes):
-        k1 = min(nz, k0 + planes)
-        w[:, k0:k1].copy_(torch.from_numpy(wl.state(k0, k1)))
+def upload_state(torch, wl, dev, planes=16, k0=0, k1=None):
+    """Generate the seeded initial state of planes [k0, k1) slab by slab on the host and place it in HBM."""
+    k1 = wl.grid["nz"] if k1 is None else k1
+    w = torch.empty((5, k1 - k0, wl.grid["ny"], wl.grid["nx"]), dtype=torch.float64, device=dev)
+    for a in range(k0, k1, planes):
+        b = min(k1, a + planes)
+        w[:, a - k0:b - k0].copy_(torch.from_numpy(wl.state(a, b)))
     return w
 
 
@@ -191,11 +196,37 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    wl = make_workload(args.config)
-    npts = wl.npoints
-    s = Streams(wl.grid, wl.x, wl.y, wl.z, wl.params, device=dev)
-    w0 = upload_state(torch, wl, dev)
-    s.set_state(w0)
+    decomp = args.decomp
+    if decomp == "auto":
+        decomp = "slab" if world > 1 and args.config in (3, 5) else ("replicas" if world > 1 else "single")
+    grp = None
+    if decomp == "slab":
+        # one z-slab of the config's size per rank; internal faces are BC_HALO (paper_2004_02276_b200/slab.py)
+        from paper_2004_02276_b200 import slab as slab_mod
+        if not dist.is_initialized():
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29577")
+            dist.init_process_group("nccl", rank=rank, world_size=world, device_id=dev)
+        glob = make_workload(args.config, zcopies=world)
+        sp = slab_mod.slab_spec(glob.grid, glob.z, glob.params, world, rank)
+        wl = glob
+        npts = sp.grid["nx"] * sp.grid["ny"] * sp.grid["nz"]
+        s = Streams(sp.grid, glob.x, glob.y, sp.z, sp.params, device=dev)
+        w0 = upload_state(torch, glob, dev, k0=sp.k0, k1=sp.k1)
+        s.set_state(w0)
+        grp = slab_mod.SlabGroup([s], world, rank=rank, periodic=True, dist=dist, forcing=bool(glob.params["forcing"]),
+                                 cfl_dt=not glob.params["dt_fixed"] > 0, overlap=not args.no_overlap)
+        do_step = grp.step
+        local_shape = (5, sp.grid["nz"], sp.grid["ny"], sp.grid["nx"])
+    else:
+        wl = make_workload(args.config)
+        npts = wl.npoints
+        s = Streams(wl.grid, wl.x, wl.y, wl.z, wl.params, device=dev)
+        w0 = upload_state(torch, wl, dev)
+        s.set_state(w0)
+        do_step = s.step
+        local_shape = wl.shape
+    del w0
     state_bytes = 5 * npts * 8
 
     def barrier():
@@ -206,7 +237,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- device-resident throughput ---------------------------------------------------------
     # exactly K steps, one streams_step(1) per step with a CUDA event between steps (no synchronisation inside the
     # timed region): the total gives `value`, the K per-step intervals give the median (median of >= 5)
-    s.step(args.warmup)
+    do_step(args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -222,7 +253,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     evs[0].record(cur)
     for i in range(args.steps):
-        s.step(1)
+        do_step(1)
         evs[i + 1].record(cur)
     barrier()
     ms = evs[0].elapsed_time(evs[-1])
@@ -230,7 +261,7 @@ def run_ours(args, rank, world, local_rank):
     launches = s.launch_count() - launches0
     if not prof_in_region:
         s.profile(True)
-        s.step(args.steps)
+        do_step(args.steps)
     rhs_ms, rhs_n = s.profile_read()
     s.profile(False)
     rhs_share = rhs_ms / (ms if prof_in_region else ms * 1.0) if ms > 0 else None
@@ -245,10 +276,10 @@ def run_ours(args, rank, world, local_rank):
     e2e = None
     if not args.no_e2e:
         try:
-            hbuf = torch.empty(wl.shape, dtype=torch.float64, pin_memory=True)
+            hbuf = torch.empty(local_shape, dtype=torch.float64, pin_memory=True)
             pinned = True
         except Exception:
-            hbuf = torch.empty(wl.shape, dtype=torch.float64)
+            hbuf = torch.empty(local_shape, dtype=torch.float64)
             pinned = False
         s.get_state_host_ptr(hbuf.data_ptr())
         ksteps = max(1, min(args.steps, args.e2e_steps))
@@ -256,7 +287,7 @@ def run_ours(args, rank, world, local_rank):
         t0 = time.perf_counter()
         for _ in range(ksteps):
             s.set_state_host_ptr(hbuf.data_ptr())      # H2D of the step's input (synchronises)
-            s.step(1)
+            do_step(1)
             s.get_state_host_ptr(hbuf.data_ptr())      # D2H of the step's result (synchronises)
         torch.cuda.synchronize(dev)
         te = time.perf_counter() - t0
@@ -268,7 +299,8 @@ def run_ours(args, rank, world, local_rank):
         stage_bytes = bytes_per_point_by_stage(wl.params)
         step_bytes = sum(stage_bytes)                                       # 448 with forcing, 400 without, +123 with WENO
         bpp = step_bytes / 3.0                                              # average k_rhs launch of a step
-        rhs_avg_ms = rhs_ms / max(rhs_n, 1)
+        n_stages = 3 * args.steps                                            # k_rhs stages profiled (a stage = 1 launch, or
+        rhs_avg_ms = rhs_ms / max(n_stages, 1)                              # interior + boundary launches on a z-slab)
         achieved = bpp * npts / (rhs_avg_ms * 1e-3) / 1e9
         traffic, traffic_src = None, None
         tpath = os.path.join(ROOT, "profiles", "k_rhs_traffic.json")
@@ -297,9 +329,14 @@ def run_ours(args, rank, world, local_rank):
                "ms_per_step": ms_max / args.steps, "ms_per_step_median": float(np.median(per_step)),
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f64", "data": "synthetic",
-               "config": {"workload": wl.name, "grid": [wl.grid["nx"], wl.grid["ny"], wl.grid["nz"]], "points": npts,
+               "config": {"workload": wl.name, "grid": list(local_shape[:0:-1]), "points": npts,
+                          "global_grid": [wl.grid["nx"], wl.grid["ny"], wl.grid["nz"]],
                           "order": wl.params["order"], "forcing": wl.params["forcing"], "weno": wl.params["weno_enable"],
-                          "parallelism": "replicas only" if world > 1 else "1 GPU",
+                          "parallelism": {"single": "1 GPU", "replicas": "replicas only (no data-path collective)",
+                                          "slab": "z-slabs, one per GPU: halo swap by NCCL send/recv overlapped with the interior chunks, "
+                                                  "all-reduce of the forcing sum per stage and of the CFL maximum per step"}[decomp],
+                          "halo_messages_per_rank_per_step": 6 if grp else 0,
+                          "halo_bytes_per_message": 7 * 3 * local_shape[2] * local_shape[3] * 8 if grp else 0,
                           "l2": "state (%.2f GB) and RK register larger than the 126 MB L2; no flush needed" % (state_bytes / 1e9)
                           if state_bytes > 2 * 126e6 else "inputs smaller than L2 (launch-latency regime)"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
@@ -326,7 +363,7 @@ def run_ours(args, rank, world, local_rank):
                "context": PAPER_CONTEXT}
         print(json.dumps(out), flush=True)
     s.close()
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 
@@ -341,6 +378,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--decomp", default="auto", choices=["auto", "single", "replicas", "slab"],
+                    help="auto: 1 GPU -> single context; N GPUs -> z-slabs (configs 3, 5), else replicas")
+    ap.add_argument("--no-overlap", action="store_true", help="slab mode: swap the halos before the whole stage kernel")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                          # timing rules: at least three warm-up steps

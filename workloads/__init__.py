@@ -193,9 +193,12 @@ def _smooth121(a, axis, periodic, passes=4):
     return a
 
 
-def config3_channel(nx=256, ny=128, nz=128, seed=1003, steps=200, name="channel", smooth=False) -> Workload:
+def config3_channel(nx=256, ny=128, nz=128, seed=1003, steps=200, name="channel", smooth=False, zcopies=1) -> Workload:
+    """zcopies > 1: a box zcopies times as long in z (nz and L_z scaled together, so the spacing stays; every plane has
+    its own noise stream): the weak-scaling input of the z-slab decomposition, nz planes per GPU (Fig. 11)."""
     gamma = 1.4
-    Lx, Lz = 6.0 * np.pi, 2.0 * np.pi
+    nz = nz * zcopies
+    Lx, Lz = 6.0 * np.pi, 2.0 * np.pi * zcopies
     x = Lx * np.arange(nx) / nx
     z = Lz * np.arange(nz) / nz
     y = tanh_nodes(ny)
@@ -239,8 +242,8 @@ def config6_channel_paper(nx=128, ny=64, nz=64, seed=1006, steps=20) -> Workload
     return wl
 
 
-def config5_channel_big(nx=1024, ny=512, nz=512, seed=1005, steps=50, smooth=False) -> Workload:
-    return config3_channel(nx, ny, nz, seed, steps, name="channel_big", smooth=smooth)
+def config5_channel_big(nx=1024, ny=512, nz=512, seed=1005, steps=50, smooth=False, zcopies=1) -> Workload:
+    return config3_channel(nx, ny, nz, seed, steps, name="channel_big", smooth=smooth, zcopies=zcopies)
 
 
 # ---------------------------------------------------------------------------------------------
