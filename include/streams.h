@@ -207,6 +207,19 @@ size_t streams_halo_bytes(const streams_ctx* ctx);
 int streams_halo_pack(streams_ctx* ctx, int face, double* d_buf, void* cuda_stream);
 int streams_halo_unpack(streams_ctx* ctx, int face, const double* d_buf, void* cuda_stream);
 
+/* The hybrid switch on z-slabs (weno_enable = 1): interface k+1/2 is flagged when any of the nodes
+ * k-2 .. k+3 has theta > theta_th (S4), so the interfaces next to a slab face need the node flags of the
+ * neighbour's three planes.  streams_stage_rhs leaves the node flags of the stage's state packed one bit per node; between
+ * streams_stage_rhs and streams_stage_end the caller swaps the flag words of the three planes next to every BC_HALO face
+ * the same way as the state halos: message [3][ny][ceil(nx/32)] 32-bit words = streams_flag_halo_bytes() bytes (0 when
+ * the switch is off).  With a frozen inflow the slab captures the inflow plane (its ghost planes included) at the first
+ * use of the state after streams_set_state, i.e. after the caller's first halo swap.  streams_rhs refuses a slab with the
+ * hybrid switch (one call cannot contain the swap); streams_sensor and the interface counts of streams_diagnostics on a
+ * slab use the ghost flag words of the last stage. */
+size_t streams_flag_halo_bytes(const streams_ctx* ctx);
+int streams_flag_halo_pack(streams_ctx* ctx, int face, unsigned int* d_buf, void* cuda_stream);
+int streams_flag_halo_unpack(streams_ctx* ctx, int face, const unsigned int* d_buf, void* cuda_stream);
+
 /* Reductions of the current state into *h_out (host struct): the volume integrals of PAPER.md:107 (bulk density
  * rho_b = 1/V int rho dV and bulk momentum, "both exactly constant in time"), total energy and kinetic energy
  * (PAPER.md:77), the last body force f, extrema and sensor statistics (Eq. 8).  Synchronises.  Returns

@@ -17,7 +17,8 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, S
 EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
            "streams_diagnostics", "streams_step_begin", "streams_stage_rhs", "streams_stage_end", "streams_reduce_ptr",
-           "streams_halo_bytes", "streams_halo_pack", "streams_halo_unpack", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
+           "streams_halo_bytes", "streams_halo_pack", "streams_halo_unpack", "streams_flag_halo_bytes", "streams_flag_halo_pack",
+           "streams_flag_halo_unpack", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
 
 
 class StreamsGrid(C.Structure):
@@ -82,6 +83,10 @@ def lib():
         L.streams_halo_bytes.restype = C.c_size_t
         L.streams_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.streams_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.streams_flag_halo_bytes.argtypes = [C.c_void_p]
+        L.streams_flag_halo_bytes.restype = C.c_size_t
+        L.streams_flag_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.streams_flag_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.streams_stats_accumulate.argtypes = [C.c_void_p]
         L.streams_stats_read.argtypes = [C.c_void_p, _DBL, C.POINTER(C.c_longlong)]
         L.streams_stats_reset.argtypes = [C.c_void_p]
@@ -310,6 +315,21 @@ class Streams:
     def halo_unpack(self, face, buf, stream=None):
         st = stream.cuda_stream if stream is not None else 0
         self._chk(lib().streams_halo_unpack(self._h, int(face), self._dev(buf, self.halo_shape()), C.c_void_p(st)))
+
+    def flag_shape(self):
+        return (3, self.n[1], (self.n[0] + 31) // 32)
+
+    def new_flag_buffer(self):
+        return self._torch.empty(self.flag_shape(), dtype=self._torch.int32, device=self.device)
+
+    def flag_halo_pack(self, face, out, stream=None):
+        st = stream.cuda_stream if stream is not None else 0
+        self._chk(lib().streams_flag_halo_pack(self._h, int(face), self._dev(out, self.flag_shape(), self._torch.int32), C.c_void_p(st)))
+        return out
+
+    def flag_halo_unpack(self, face, buf, stream=None):
+        st = stream.cuda_stream if stream is not None else 0
+        self._chk(lib().streams_flag_halo_unpack(self._h, int(face), self._dev(buf, self.flag_shape(), self._torch.int32), C.c_void_p(st)))
 
     def diagnostics(self, check=True):
         d = StreamsDiag()

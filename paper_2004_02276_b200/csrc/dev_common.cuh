@@ -36,7 +36,7 @@ struct DevP {
   long long N;                       // nx*ny*nz
   long long QS;                      // doubles between two fields of a primitive-state buffer: (nz + 2 zpad) * nxy
   int zpad;                          // ghost planes stored below / above the state (3 when a z face is BC_HALO, else 0)
-  int pad_;
+  int IS;                            // doubles between two fields of the frozen inflow plane: (nz + 2 zpad) * ny
   double gam, gm1, Rgas, inv_R, cp, cv, inv_cv, cp_over_Pr;
   double mu_ref, T_ref, inv_Tref, visc_exp, suth_S;
   double th_thr, th_eps;
@@ -200,7 +200,7 @@ __device__ __forceinline__ void load_src_raw(const DevP& P, const double* __rest
     q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.QS); q.v = __ldg(Q + o + 2 * P.QS); q.w = __ldg(Q + o + 3 * P.QS);
     q.T = __ldg(Q + o + 4 * P.QS); q.mu = __ldg(Q + o + 5 * P.QS); q.H = __ldg(Q + o + 6 * P.QS);
   } else if (k == SRC_INFLOW) {
-    const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
+    const long long o = (long long)kk * P.ny + s.off, st = P.IS;
     q.rho = P.inflow[o]; q.u = P.inflow[o + st]; q.v = P.inflow[o + 2 * st]; q.w = P.inflow[o + 3 * st];
     q.T = P.inflow[o + 4 * st]; q.mu = P.inflow[o + 5 * st]; q.H = P.inflow[o + 6 * st];
   } else {
@@ -227,7 +227,7 @@ __device__ __forceinline__ void fetch_prim5(const DevP& P, const double* __restr
     const long long o = (long long)kk * P.nxy + s.off;
     q.rho = __ldg(Q + o); q.u = __ldg(Q + o + P.QS); q.v = __ldg(Q + o + 2 * P.QS); q.w = __ldg(Q + o + 3 * P.QS); q.T = __ldg(Q + o + 4 * P.QS);
   } else if (kd == SRC_INFLOW) {
-    const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
+    const long long o = (long long)kk * P.ny + s.off, st = P.IS;
     q.rho = P.inflow[o]; q.u = P.inflow[o + st]; q.v = P.inflow[o + 2 * st]; q.w = P.inflow[o + 3 * st]; q.T = P.inflow[o + 4 * st];
   } else {
     const double* c = kd == SRC_POST ? P.post : P.fs;
@@ -249,7 +249,7 @@ __device__ __forceinline__ void fetch_vel(const DevP& P, const double* __restric
     const long long o = (long long)kk * P.nxy + s.off;
     u = __ldg(Q + o + P.QS); v = __ldg(Q + o + 2 * P.QS); w = __ldg(Q + o + 3 * P.QS);
   } else if (kd == SRC_INFLOW) {
-    const size_t o = (size_t)kk * P.ny + s.off, st = (size_t)P.nz * P.ny;
+    const long long o = (long long)kk * P.ny + s.off, st = P.IS;
     u = P.inflow[o + st]; v = P.inflow[o + 2 * st]; w = P.inflow[o + 3 * st];
   } else {
     const double* c = kd == SRC_POST ? P.post : P.fs;

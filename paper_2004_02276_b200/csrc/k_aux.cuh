@@ -264,13 +264,14 @@ __global__ void __launch_bounds__(1024) k_fp64_peak(double* __restrict__ out, in
   if (r == 123.456) out[0] = r;              // never true: keeps the chains alive
 }
 
-// capture the frozen inflow plane (S1 INFLOW_FROZEN): inflow[v][k][j] = Q[v][k][j][0]
+// capture the frozen inflow plane (S1 INFLOW_FROZEN): inflow[v][k][j] = Q[v][k][j][0], all stored planes k (a z-slab
+// keeps the ghost planes of the inflow as well: k = -zpad .. nz + zpad - 1; `Q` and `inflow` point at plane 0)
 __global__ void k_capture_inflow(const __grid_constant__ DevP P, const double* __restrict__ Q, double* __restrict__ inflow) {
-  const long long n = (long long)P.nz * P.ny;
+  const long long n = P.IS, r0 = -(long long)P.zpad * P.ny;
   for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < NQ * n; e += (long long)gridDim.x * blockDim.x) {
     const int v = (int)(e / n);
-    const long long r = e % n;
-    inflow[e] = Q[v * P.QS + r * P.nx];
+    const long long r = r0 + e % n;
+    inflow[v * n + r] = Q[v * P.QS + r * P.nx];
   }
 }
 

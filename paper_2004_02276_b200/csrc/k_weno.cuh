@@ -89,10 +89,13 @@ __device__ __forceinline__ unsigned int xbit(const DevP& P, const unsigned int* 
   const int ii = P.bc[0] == BC_PERIODIC ? wrap(i, P.nx) : min(max(i, 0), P.nx - 1);
   return (rw[ii >> 5] >> (ii & 31)) & 1u;
 }
-// row index of (j, k) with the ghost rule of the sensor along y / z
+// row index of (j, k) with the ghost rule of the sensor along y / z; beyond a BC_HALO face the row is one of the
+// neighbouring slab's (stored around the flag words like the ghost planes around the state: negative / >= nz*ny)
 __device__ __forceinline__ int row_of(const DevP& P, int j, int k) {
   const int jj = P.bc[2] == BC_PERIODIC ? wrap(j, P.ny) : min(max(j, 0), P.ny - 1);
-  const int kk = P.bc[4] == BC_PERIODIC ? wrap(k, P.nz) : min(max(k, 0), P.nz - 1);
+  int kk = k;
+  if (k < 0) kk = P.bc[4] == BC_PERIODIC ? wrap(k, P.nz) : (P.bc[4] == BC_HALO ? k : 0);
+  else if (k >= P.nz) kk = P.bc[5] == BC_PERIODIC ? wrap(k, P.nz) : (P.bc[5] == BC_HALO ? k : P.nz - 1);
   return kk * P.ny + jj;
 }
 
@@ -150,8 +153,8 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
         unsigned int wy[7], wz[7];
 #pragma unroll
         for (int g = 0; g < 7; ++g) {
-          wy[g] = fbits[(size_t)row_of(P, j - 3 + g, k) * nw + wi];
-          wz[g] = fbits[(size_t)row_of(P, j, k - 3 + g) * nw + wi];
+          wy[g] = fbits[(long long)row_of(P, j - 3 + g, k) * nw + wi];
+          wz[g] = fbits[(long long)row_of(P, j, k - 3 + g) * nw + wi];
         }
         lo[1] = wy[0] | wy[1] | wy[2] | wy[3] | wy[4] | wy[5]; hi[1] = wy[1] | wy[2] | wy[3] | wy[4] | wy[5] | wy[6];
         lo[2] = wz[0] | wz[1] | wz[2] | wz[3] | wz[4] | wz[5]; hi[2] = wz[1] | wz[2] | wz[3] | wz[4] | wz[5] | wz[6];
@@ -232,7 +235,11 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
   }
 }
 
-__device__ __forceinline__ double weno5(double a, double b, double c, double d, double e) {
+// WENO5-JS reconstruction (ref. [34]) as numerator and denominator: value = num / den.
+// Weights a_k = d_k / (eps + b_k)^2 written over the common denominator e0 e1 e2: w_k = d_k prod_{j != k} e_j,
+// value = sum w_k q_k / sum w_k.  The caller adds the upwind and the downwind reconstruction of a characteristic field
+// over ONE division: n+/d+ + n-/d- = (n+ d- + n- d+) / (d+ d-)  (one division per field instead of four in the textbook form).
+__device__ __forceinline__ void weno5_nd(double a, double b, double c, double d, double e, double& num, double& den) {
   const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) * (1.0 / 6.0);
   const double q1 = (-b + 5.0 * c + 2.0 * d) * (1.0 / 6.0);
   const double q2 = (2.0 * c + 5.0 * d - e) * (1.0 / 6.0);
@@ -242,12 +249,11 @@ __device__ __forceinline__ double weno5(double a, double b, double c, double d, 
   const double b0 = (13.0 / 12.0) * t0 * t0 + 0.25 * u0 * u0;
   const double b1 = (13.0 / 12.0) * t1 * t1 + 0.25 * u1 * u1;
   const double b2 = (13.0 / 12.0) * t2 * t2 + 0.25 * u2 * u2;
-  // WENO-JS weights a_k = d_k / (eps + b_k)^2 (ref. [34]), written over the common denominator e0 e1 e2 so that the
-  // interface costs one division instead of four: w_k = d_k prod_{j != k} e_j, result = sum w_k q_k / sum w_k
   const double eps = 1e-6;
   const double e0 = (eps + b0) * (eps + b0), e1 = (eps + b1) * (eps + b1), e2 = (eps + b2) * (eps + b2);
   const double a0 = 0.1 * (e1 * e2), a1 = 0.6 * (e0 * e2), a2 = 0.3 * (e0 * e1);
-  return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
+  num = a0 * q0 + a1 * q1 + a2 * q2;
+  den = a0 + a1 + a2;
 }
 
 // dF = F_weno - F_central at the interface between node (i,j,k) and its upper neighbour along D (S5, S6)
@@ -323,7 +329,12 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
     double fp[6], fm[6];
 #pragma unroll
     for (int n = 0; n < 6; ++n) { fp[n] = 0.5 * (fc[n][s] + al[s] * wc[n][s]); fm[n] = 0.5 * (fc[n][s] - al[s] * wc[n][s]); }
-    fh[s] = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+    double np_, dp_, nm_, dm_;
+    weno5_nd(fp[0], fp[1], fp[2], fp[3], fp[4], np_, dp_);
+    weno5_nd(fm[5], fm[4], fm[3], fm[2], fm[1], nm_, dm_);
+    // range: den ~ (eps + beta)^4 with beta ~ F^2 (F = characteristic flux), so d+ d- ~ F^16 between 1e-48 (smooth
+    // data, eps^8) and fp64 overflow at F ~ 1e19: no rescaling needed in any sensible unit system
+    fh[s] = (np_ * dm_ + nm_ * dp_) / (dp_ * dm_);
   }
   // step 7: back to conservative variables
   double Fw[5];

@@ -55,6 +55,7 @@ struct streams_ctx {
   int zpad;                            // ghost planes stored around each state buffer (3 with a BC_HALO z face)
   int stage_next;                      // staged stepping: -1 = between steps, else the stage whose streams_stage_rhs /
   int stage_half;                      // streams_stage_end comes next (half: 0 = rhs pending, 1 = end pending)
+  int inflow_pending;                  // z-slab with INFLOW_FROZEN: the frozen plane is captured once the ghost planes are in
   int parts_done;                      // bit 0: interior chunks launched, bit 1: boundary chunks launched (this stage)
   CUtensorMap tmap[2];           // TMA descriptors of qbuf[0], qbuf[1] as 4-D tensors (x, y, z, field)
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
@@ -145,7 +146,6 @@ const char* validate(const streams_grid* g, const streams_params* p) {
   if (p->forcing && p->bc[0] != STREAMS_BC_PERIODIC) return "bulk forcing needs a periodic x direction";
   if (p->bc[4] == STREAMS_BC_HALO || p->bc[5] == STREAMS_BC_HALO) {
     if (p->weno_enable && p->forcing) return "z-slabs: forcing and the hybrid switch together are not supported";
-    if (p->bc[0] == STREAMS_BC_INFLOW_FROZEN) return "z-slabs: INFLOW_FROZEN is not supported (the frozen plane has no ghost planes)";
   }
   return nullptr;
 }
@@ -227,7 +227,7 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   if (p.weno_enable) {
     L.theta = c.take(N * sizeof(double));
     L.nflag = c.take(N);
-    L.fbits = c.take((size_t)g.ny * g.nz * ((g.nx + 31) / 32) * sizeof(unsigned int));
+    L.fbits = c.take((size_t)g.ny * (g.nz + 2 * L.zpad) * ((g.nx + 31) / 32) * sizeof(unsigned int));
     L.lmask = c.take(N);
     L.list = c.take(N * sizeof(unsigned int));
     L.istride = N + std::max({(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny});
@@ -265,7 +265,7 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   L.grid = dim3(tiles_x, tiles_y, nchunk);
   L.npartial = std::max(tiles * nchunk, NDIAG * RGRID);
   L.partial = c.take((size_t)L.npartial * sizeof(double));
-  L.inflow = c.take((size_t)NQ * g.nz * g.ny * sizeof(double));
+  L.inflow = c.take((size_t)NQ * (g.nz + 2 * L.zpad) * g.ny * sizeof(double));
   L.speeds = c.take(8 * sizeof(double));
   L.sc = c.take(sizeof(DevScal));        // device scalars in caller memory: the caller may run collectives on streams_reduce_ptr
   L.total = c.off;
@@ -381,10 +381,10 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]) + zoff; c->S[i] = (double*)(base + L.S[i]); }
   if (p->weno_enable) {
     c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
-    c->fbits = (unsigned int*)(base + L.fbits); c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
+    c->fbits = (unsigned int*)(base + L.fbits) + (size_t)L.zpad * g->ny * ((g->nx + 31) / 32); c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
     c->ilist = (unsigned int*)(base + L.ilist); c->dFbuf = (double*)(base + L.dFbuf); c->dFb = (double*)(base + L.dFb);
   }
-  c->partial = (double*)(base + L.partial); c->inflow = (double*)(base + L.inflow); c->speeds = (double*)(base + L.speeds);
+  c->partial = (double*)(base + L.partial); c->inflow = (double*)(base + L.inflow) + (size_t)L.zpad * g->ny; c->speeds = (double*)(base + L.speeds);
   c->npartial = L.npartial; c->rhs_grid = L.grid; c->lz = L.lz; c->istride = L.istride;
   c->sc = (DevScal*)(base + L.sc);
   c->stage_next = -1;
@@ -446,7 +446,7 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   // ---- device parameter block ----
   DevP& P = c->P;
   P.nx = n[0]; P.ny = n[1]; P.nz = n[2]; P.nxy = n[0] * n[1]; P.N = (long long)n[0] * n[1] * n[2];
-  P.zpad = L.zpad; P.QS = (long long)n[0] * n[1] * (n[2] + 2 * L.zpad);
+  P.zpad = L.zpad; P.QS = (long long)n[0] * n[1] * (n[2] + 2 * L.zpad); P.IS = n[1] * (n[2] + 2 * L.zpad);
   for (int i = 0; i < 6; ++i) P.bc[i] = p->bc[i];
   P.visc_model = p->visc_model; P.weno = p->weno_enable; P.forcing = p->forcing; P.viscous = p->viscous_enable; P.L = p->order / 2;
   P.gam = p->gamma; P.gm1 = p->gamma - 1.0; P.Rgas = p->Rgas; P.inv_R = 1.0 / p->Rgas;
@@ -521,9 +521,11 @@ static int after_set_state(streams_ctx* c, const double* d_w) {
   c->cur = 0;
   k_cons2prim<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, d_w, c->qbuf[0]);
   LAUNCH_CHECK("k_cons2prim");
+  c->inflow_pending = 0;
   if (c->p.bc[0] == STREAMS_BC_INFLOW_FROZEN) {
-    k_capture_inflow<<<64, 256, 0, c->st>>>(c->P, c->qbuf[0], c->inflow);
-    LAUNCH_CHECK("k_capture_inflow");
+    // a z-slab freezes its ghost planes of the inflow as well: they arrive with the first halo swap (ensure_inflow)
+    if (c->zpad) c->inflow_pending = 1;
+    else { k_capture_inflow<<<64, 256, 0, c->st>>>(c->P, c->qbuf[0], c->inflow); LAUNCH_CHECK("k_capture_inflow"); }
   }
   // keep vol_total: reset the other scalars one by one
   CK(cudaMemsetAsync(&c->sc->force, 0, sizeof(double), c->st));
@@ -586,12 +588,27 @@ static int run_sensor(streams_ctx* c, const double* w, double* theta_out, unsign
   return STREAMS_OK;
 }
 
-// list of nodes with flagged interfaces from the node flags k_rhs has just written (a3)
+// z-slab with a frozen inflow: capture the inflow plane (ghost planes included) the first time the state is used after
+// set_state -- the caller has swapped the halos of the initial state by then (include/streams.h)
+static int ensure_inflow(streams_ctx* c) {
+  if (!c->inflow_pending) return STREAMS_OK;
+  k_capture_inflow<<<64, 256, 0, c->st>>>(c->P, c->qbuf[c->cur], c->inflow);
+  LAUNCH_CHECK("k_capture_inflow");
+  c->inflow_pending = 0;
+  return STREAMS_OK;
+}
+
+// node flags k_rhs has just written -> one bit per node (a3).  On a z-slab the caller now swaps the flag words of the
+// three planes next to each BC_HALO face (streams_flag_halo_*) before run_list.
+static int run_flag_pack(streams_ctx* c) {
+  k_flag_pack<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->fbits);
+  LAUNCH_CHECK("k_flag_pack");
+  return STREAMS_OK;
+}
+// lists of flagged interfaces and of the nodes next to them from the packed flags
 static int run_list(streams_ctx* c) {
   CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
   CK(cudaMemsetAsync(&c->sc->icount[0], 0, 4 * sizeof(unsigned int), c->st));
-  k_flag_pack<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->fbits);
-  LAUNCH_CHECK("k_flag_pack");
   k_weno_list<<<wgrid_for(c), RT, 0, c->st>>>(c->P, c->fbits, c->list, c->lmask, c->ilist, c->istride, nullptr, c->sc);
   LAUNCH_CHECK("k_weno_list");
   return STREAMS_OK;
@@ -647,8 +664,10 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   if (!c || !d_rhs) return fail(c, STREAMS_EINVAL, "null argument");
   DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
+  if (c->zpad && c->p.weno_enable) return fail(c, STREAMS_EINVAL, "streams_rhs on a z-slab with the hybrid switch: the flag words are swapped between the staged calls");
   const double* w = c->qbuf[c->cur];
   int rc;
+  if ((rc = ensure_inflow(c))) return rc;
   RhsArgs A;
   std::memset(&A, 0, sizeof A);
   A.q = w; A.out_rhs = d_rhs; A.lz = c->lz; A.cz0 = 0; A.czs = 1;
@@ -656,6 +675,7 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   A.partial = partial_ok ? c->partial : nullptr;
   if ((rc = launch_rhs(c, 0, A, c->rhs_grid))) return rc;
   if (c->p.weno_enable) {
+    if ((rc = run_flag_pack(c))) return rc;
     if ((rc = run_weno(c, w, d_rhs, nullptr, 0.0))) return rc;
   }
   if (c->p.forcing) {
@@ -671,6 +691,7 @@ int streams_sensor(streams_ctx* c, double* d_theta, unsigned char* d_flags) {
   DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   if (!c->p.weno_enable) return fail(c, STREAMS_EINVAL, "streams_sensor needs weno_enable = 1");
+  if (int rc = ensure_inflow(c)) return rc;
   return run_sensor(c, c->qbuf[c->cur], d_theta, d_flags, false);
 }
 
@@ -708,6 +729,7 @@ static bool part_chunks(const streams_ctx* c, int part, RhsArgs& A, dim3& grid) 
 static int do_stage_rhs(streams_ctx* c, int l, int part, bool single) {
   int rc;
   const bool first = part != PART_BOUNDARY, last = part != PART_INTERIOR;
+  if (first && (rc = ensure_inflow(c))) return rc;
   if (l == 0 && first && !(c->p.dt_fixed > 0.0)) {
     k_take_dt<<<1, 1, 0, c->st>>>(c->sc, c->p.cfl);
     LAUNCH_CHECK("k_take_dt");
@@ -732,10 +754,12 @@ static int do_stage_rhs(streams_ctx* c, int l, int part, bool single) {
     const bool partial_ok = !c->p.weno_enable;
     A.out_rhs = c->S[c->scur ^ 1]; A.partial = partial_ok ? c->partial : nullptr;
     if (any && (rc = launch_rhs(c, 0, A, grid))) return rc;
+    if (last && c->p.weno_enable && (rc = run_flag_pack(c))) return rc;
   } else {
     // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
     A.q_out = c->qbuf[c->cur ^ 1]; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
     if (any && (rc = launch_rhs(c, 1, A, grid))) return rc;
+    if (last && c->p.weno_enable && (rc = run_flag_pack(c))) return rc;
   }
   return STREAMS_OK;
 }
@@ -896,6 +920,27 @@ static int halo_copy(streams_ctx* c, int face, double* buf, void* stream, bool p
   }
   return STREAMS_OK;
 }
+// node-flag words (one bit per node) of the three planes next to a z face <-> a contiguous message [3][ny][ceil(nx/32)]
+static int flag_halo_copy(streams_ctx* c, int face, unsigned int* buf, void* stream, bool pack) {
+  if (!c || !buf || (face != 4 && face != 5)) return fail(c, STREAMS_EINVAL, "bad argument (face: 4 = zmin, 5 = zmax)");
+  DevGuard dg(c->device);
+  if (!c->p.weno_enable) return fail(c, STREAMS_EINVAL, "flag halos need weno_enable = 1");
+  if (!pack && c->p.bc[face] != STREAMS_BC_HALO) return fail(c, STREAMS_EINVAL, "streams_flag_halo_unpack: this face is not BC_HALO");
+  cudaStream_t st = stream ? (cudaStream_t)stream : c->st;
+  const long long k = pack ? (face == 4 ? 0 : c->P.nz - HALO) : (face == 4 ? -HALO : c->P.nz);
+  const size_t rowwords = (size_t)c->P.ny * ((c->P.nx + 31) / 32), n = HALO * rowwords;
+  unsigned int* f = c->fbits + k * (long long)rowwords;
+  if (pack) CK(cudaMemcpyAsync(buf, f, n * sizeof(unsigned int), cudaMemcpyDeviceToDevice, st));
+  else CK(cudaMemcpyAsync(f, buf, n * sizeof(unsigned int), cudaMemcpyDeviceToDevice, st));
+  return STREAMS_OK;
+}
+size_t streams_flag_halo_bytes(const streams_ctx* c) {
+  return c && c->p.weno_enable ? (size_t)HALO * c->P.ny * ((c->P.nx + 31) / 32) * sizeof(unsigned int) : 0;
+}
+int streams_flag_halo_pack(streams_ctx* c, int face, unsigned int* d_buf, void* cuda_stream) { return flag_halo_copy(c, face, d_buf, cuda_stream, true); }
+int streams_flag_halo_unpack(streams_ctx* c, int face, const unsigned int* d_buf, void* cuda_stream) {
+  return flag_halo_copy(c, face, const_cast<unsigned int*>(d_buf), cuda_stream, false);
+}
 int streams_halo_pack(streams_ctx* c, int face, double* d_buf, void* cuda_stream) { return halo_copy(c, face, d_buf, cuda_stream, true); }
 int streams_halo_unpack(streams_ctx* c, int face, const double* d_buf, void* cuda_stream) {
   return halo_copy(c, face, const_cast<double*>(d_buf), cuda_stream, false);
@@ -943,6 +988,7 @@ int streams_diagnostics(streams_ctx* c, streams_diag* out) {
   const int rg = rgrid_for(c->P.N);
   const double* w = c->qbuf[c->cur];
   int rc;
+  if ((rc = ensure_inflow(c))) return rc;
   // sensor statistics of the current state (interface counts as the next RHS would see them)
   if (c->p.weno_enable && (rc = run_sensor(c, w, nullptr, nullptr, false))) return rc;
   DevScal& hs = *c->h_sc;

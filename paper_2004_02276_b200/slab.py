@@ -4,13 +4,14 @@ Host-side orchestration only.  Every slab is one context of the CUDA library who
 `BC_HALO`; all arithmetic runs in the library's kernels through the staged C-ABI calls (include/streams.h):
 
     step_begin | MAX of red[2] | for each stage: swap halos, stage_rhs(interior) while the swap is in flight,
-    stage_rhs(boundary), SUM of red[0..1] (forcing), stage_end.
+    stage_rhs(boundary), SUM of red[0..1] (forcing), swap of the node-flag words (hybrid switch), stage_end.
 
 The messages move by `torch.distributed` point-to-point operations between processes (NCCL on GPUs, one process per
 GPU) and by device-to-device copies between slabs of the same process.
 
 A "slab" is duck-typed (binding.Streams provides it): `halo_pack(face, out, stream)`, `halo_unpack(face, buf, stream)`,
-`step_begin()`, `stage_rhs(stage, part)`, `stage_end(stage)`, `red`, `stream`, `halo_shape()`, `new_buffer()`; the
+`step_begin()`, `stage_rhs(stage, part)`, `stage_end(stage)`, `red`, `stream`, `halo_shape()`, `new_buffer()` (and
+`flag_halo_pack/unpack`, `new_flag_buffer()` with the hybrid switch); the
 stream handling is delegated to a small `Sync` object so that the CPU (gloo) tests can run the same logic on NumPy /
 CPU-tensor slabs.
 """
@@ -171,7 +172,7 @@ class SlabGroup:
     is then a local copy).  `reducer` combines the partial reductions (DistReducer, or a test's own)."""
 
     def __init__(self, slabs, nslabs, rank=0, periodic=True, dist=None, group=None, reducer=None, syncs=None,
-                 forcing=False, cfl_dt=True, overlap=True):
+                 forcing=False, cfl_dt=True, overlap=True, weno=False):
         self.slabs = list(slabs)
         K = len(self.slabs)
         if K < 1 or nslabs % K:
@@ -195,6 +196,10 @@ class SlabGroup:
         self.sbuf = {f: [s.new_buffer() for s in self.slabs] for f in (FACE_ZMIN, FACE_ZMAX)}
         self.rbuf = {FACE_ZMIN: self.slabs[0].new_buffer(), FACE_ZMAX: self.slabs[-1].new_buffer()}
         self._consumed = [[] for _ in range(K)]      # events of the unpacks that read slab i's send buffers
+        self.weno = bool(weno)
+        if self.weno:                                # node-flag words of the hybrid switch: a second, small message per face
+            self.fsbuf = {f: [s.new_flag_buffer() for s in self.slabs] for f in (FACE_ZMIN, FACE_ZMAX)}
+            self.frbuf = {FACE_ZMIN: self.slabs[0].new_flag_buffer(), FACE_ZMAX: self.slabs[-1].new_flag_buffer()}
         self.messages_sent = 0                       # bench / test accounting (messages that left a slab)
 
     # -- helpers
@@ -209,6 +214,15 @@ class SlabGroup:
     def swap_halos(self):
         """Pack, move and unpack the ghost planes of the current state of every local slab; returns one event per
         slab after which its ghost planes are in place (None on CPU)."""
+        return self._swap("halo_pack", "halo_unpack", self.sbuf, self.rbuf)
+
+    def swap_flags(self):
+        """The same for the node-flag words of the hybrid switch (between stage_rhs and stage_end); the context
+        streams wait for it."""
+        for i, ev in enumerate(self._swap("flag_halo_pack", "flag_halo_unpack", self.fsbuf, self.frbuf)):
+            self.syncs[i].main_wait(ev)
+
+    def _swap(self, pack, unpack, sbuf, rbuf):
         K = len(self.slabs)
         sy = self.syncs
         packed = []
@@ -219,9 +233,9 @@ class SlabGroup:
             self._consumed[i] = []
             lo, hi = self.nb[i]
             if lo is not None:
-                s.halo_pack(FACE_ZMIN, self.sbuf[FACE_ZMIN][i], stream=sy[i].comm)
+                getattr(s, pack)(FACE_ZMIN, sbuf[FACE_ZMIN][i], stream=sy[i].comm)
             if hi is not None:
-                s.halo_pack(FACE_ZMAX, self.sbuf[FACE_ZMAX][i], stream=sy[i].comm)
+                getattr(s, pack)(FACE_ZMAX, sbuf[FACE_ZMAX][i], stream=sy[i].comm)
             packed.append(sy[i].comm_done())
         # messages between slabs of this process (incl. the periodic seam when this process holds every slab)
         via_dist = self.dist is not None and (self.world > 1 or K == 1)
@@ -235,7 +249,7 @@ class SlabGroup:
                 crosses = via_dist and ((face == FACE_ZMIN and i == 0) or (face == FACE_ZMAX and i == K - 1))
                 if j is not None and not crosses:
                     sy[i].comm_wait(packed[j])
-                    s.halo_unpack(face, self.sbuf[src_face][j], stream=sy[i].comm)
+                    getattr(s, unpack)(face, sbuf[src_face][j], stream=sy[i].comm)
                     self._consumed[j].append(sy[i].comm_done())
                     self.messages_sent += 1
                 else:
@@ -254,18 +268,18 @@ class SlabGroup:
                 for face in (FACE_ZMAX, FACE_ZMIN):
                     if face in remote:
                         i, peer = remote[face]
-                        p2p.append(dist.P2POp(dist.isend, self.sbuf[face][i], peer, group=self.group))
+                        p2p.append(dist.P2POp(dist.isend, sbuf[face][i], peer, group=self.group))
                 for face in (FACE_ZMIN, FACE_ZMAX):
                     if face in remote:
                         i, peer = remote[face]
-                        p2p.append(dist.P2POp(dist.irecv, self.rbuf[face], peer, group=self.group))
+                        p2p.append(dist.P2POp(dist.irecv, rbuf[face], peer, group=self.group))
                 for w in dist.batch_isend_irecv(p2p):
                     w.wait()
                 self.messages_sent += len(remote)
                 done = sy[0].comm_done()
             for face, (i, peer) in remote.items():
                 sy[i].comm_wait(done)
-                self.slabs[i].halo_unpack(face, self.rbuf[face], stream=sy[i].comm)
+                getattr(self.slabs[i], unpack)(face, rbuf[face], stream=sy[i].comm)
         return [sy[i].comm_done() for i in range(K)]
 
     def step(self, nsteps=1):
@@ -285,6 +299,8 @@ class SlabGroup:
                     s.stage_rhs(stage, PART_BOUNDARY if self.overlap else PART_ALL)
                 if self.forcing and self.combine:
                     self.reducer.sum(sl, sy)
+                if self.weno:
+                    self.swap_flags()
                 for s in sl:
                     s.stage_end(stage)
 

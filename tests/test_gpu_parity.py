@@ -103,10 +103,13 @@ def check_rhs(env, wl, tol=RHS_TOL):
 
 
 def check_flags(env, o, g, sync=False):
-    """theta to 1e-12 and interface flags exactly, on the SAME state (sync=True first hands the oracle's
-    current state to the GPU context: after independent runs the two states differ at the 1e-10 level)."""
+    """theta to 1e-12 and interface flags exactly, on the SAME state (sync=True first hands the oracle's current
+    state to BOTH sides: after independent runs the two states differ at the 1e-10 level, and set_state freezes the
+    inflow plane of an INFLOW_FROZEN case anew, which must happen on both sides)."""
     if sync:
-        g.set_state(env[0].from_numpy(o.get_state()).cuda())
+        w = o.get_state()
+        o.set_state(w)
+        g.set_state(env[0].from_numpy(w).cuda())
     th_o, fl_o = o.sensor()
     th_g, fl_g = g.sensor()
     # theta = -div / sqrt(div^2 + |curl|^2 + eps): a velocity rounding error delta gives |d theta| <= delta/(h sqrt(eps));

@@ -243,3 +243,38 @@ def test_nccl_self_exchange_world_size_one(env):
         if created:
             dist.destroy_process_group()
     one.close()
+
+
+@pytest.mark.parametrize("case", ["weno_box", "sbli"])
+def test_hybrid_switch_on_slabs_is_bitwise_the_undivided_run(env, case):
+    """The hybrid switch across slab faces: the node-flag words of the neighbour's three planes are
+    swapped between stage_rhs and stage_end; the interfaces next to a face are then flagged, listed and corrected exactly as
+    in the undivided run.  `sbli` adds the frozen inflow (captured with its ghost planes after the first halo swap), the
+    node wall, the shock generator and the characteristic outflow."""
+    torch, binding, slab, ob = env
+    if case == "weno_box":
+        wl = W.random_periodic(32, 16, 36, params=W.default_params(Rgas=1 / 1.4, mu_ref=5e-3, weno_enable=1,
+                                                                   sensor_threshold=0.3, sensor_eps=0.1))
+        nsl = 3
+    else:
+        wl = W.config4_sbli(64, 40, 16)
+        nsl = 2
+    w0 = wl.state()
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(w0).cuda())
+    one.step(3)
+    ref = one.get_state().cpu().numpy()
+    d1 = one.diagnostics()
+    assert sum(d1.weno_ifaces) > 0, "the case must exercise the WENO branch"
+    ctxs, specs, _ = make_slabs(env, wl, nsl)
+    grp = slab.SlabGroup(ctxs, nsl, periodic=True, reducer=HostReducer(torch), forcing=False, cfl_dt=True, weno=True)
+    grp.step(3)
+    got = gather(ctxs)
+    assert np.array_equal(got, ref), np.abs(got - ref).max()
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    o.set_state(w0)
+    o.step(3)
+    assert l2(got, o.get_state()) < STEP_TOL
+    for c in ctxs + [one]:
+        c.close()
+    o.close()
