@@ -278,3 +278,66 @@ def test_hybrid_switch_on_slabs_is_bitwise_the_undivided_run(env, case):
     for c in ctxs + [one]:
         c.close()
     o.close()
+
+
+def test_config5_size_two_slabs_one_step_bitwise(env):
+    """The 1024x512x512 channel block (config 5: 32 x 64 tiles, wall tiles, lazy forcing, four 128-plane chunks) cut into
+    two 1024x512x256 slabs on the same device, in the launch configuration bench.py --decomp slab times (interior chunks
+    while the halos move, boundary chunks after): one RK3 step, fed reductions, bit for bit the undivided context."""
+    torch, binding, slab, _ = env
+    wl = W.config5_channel_big()
+    nz, planes = wl.grid["nz"], 32
+
+    def upload(ctx, k0, k1):
+        w = torch.empty((5, k1 - k0, wl.grid["ny"], wl.grid["nx"]), dtype=torch.float64, device="cuda")
+        for a in range(k0, k1, planes):
+            b = min(k1, a + planes)
+            w[:, a - k0:b - k0].copy_(torch.from_numpy(wl.state(a, b)))
+        ctx.set_state(w)
+        del w
+
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    upload(one, 0, nz)
+    ctxs, specs = [], []
+    for r in range(2):
+        sp = slab.slab_spec(wl.grid, wl.z, wl.params, 2, r)
+        c = binding.Streams(sp.grid, wl.x, wl.y, sp.z, sp.params)
+        upload(c, sp.k0, sp.k1)
+        ctxs.append(c)
+        specs.append(sp)
+    grp = slab.SlabGroup(ctxs, 2, periodic=True, reducer=HostReducer(torch), forcing=True)
+
+    def feed(lo, hi):
+        one.stream.synchronize()
+        v = one.red[lo:hi].clone()
+        for c in ctxs:
+            with torch.cuda.stream(c.stream):
+                c.red[lo:hi].copy_(v)
+            c.stream.synchronize()
+
+    one.step_begin()
+    for c in ctxs:
+        c.step_begin()
+    feed(2, 3)
+    for stage in range(3):
+        ready = grp.swap_halos()
+        one.stage_rhs(stage, one.PART_ALL)
+        for c in ctxs:
+            c.stage_rhs(stage, c.PART_INTERIOR)
+        for i, c in enumerate(ctxs):
+            grp.syncs[i].main_wait(ready[i])
+            c.stage_rhs(stage, c.PART_BOUNDARY)
+        feed(0, 2)
+        one.stage_end(stage)
+        for c in ctxs:
+            c.stage_end(stage)
+    ref = one.get_state()
+    for c, sp in zip(ctxs, specs):
+        got = c.get_state()
+        assert torch.equal(got, ref[:, sp.k0:sp.k1]), float((got - ref[:, sp.k0:sp.k1]).abs().max())
+        del got
+    d = [c.diagnostics() for c in ctxs + [one]]
+    assert d[0].dt == d[2].dt and d[0].forcing == d[2].forcing and d[1].forcing == d[2].forcing
+    assert abs(d[0].mass + d[1].mass - d[2].mass) <= 1e-12 * d[2].mass
+    for c in ctxs + [one]:
+        c.close()
