@@ -487,8 +487,11 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     const int buf = it & 1;                              // tile buffer of plane s; its mbarrier is in phase (it >> 1) & 1
     const unsigned phase = (unsigned)(it >> 1) & 1u;
     double* t = tiles + buf * SM_TILE1;
+    // Addresses: a warp-uniform pointer (plane, field) plus the node's 32-bit offset inside a plane (two instructions per
+    // address; a 64-bit per-thread element index costs four, and the loop forms 24 addresses per plane)
+    const unsigned own32 = (unsigned)own_off;
     if (active && s + 5 < k1 + 3) {
-      const double* q = A.q + own_off + (long long)map_z(P, s + 5) * P.nxy;
+      const double* q = (A.q + (long long)map_z(P, s + 5) * P.nxy) + own32;
       const unsigned d = smem_u32(oring + tid) + ((b3 == 0 ? 2 : b3 - 1) * NF * NPT) * 8;       // (it + 5) % 3
 #pragma unroll
       for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.QS);
@@ -496,11 +499,12 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     if (FUSED && A.alpha != 0.0 && active && s - 2 >= k0 && s - 2 < k1) {
       // R_prev (and u_prev for the lazy forcing) of plane s-2, read in the NEXT step's epilogue (one step of slack:
       // the epilogue sits before the plane barrier and must not wait for HBM)
-      const size_t o = (size_t)(s - 2) * P.nxy + own_off;
+      const long long zo = (long long)(s - 2) * P.nxy;
+      const double* sp = (A.S_prev + zo) + own32;
       const unsigned d = smem_u32(spring + tid) + (((it + 1) & 1) * 6 * NPT) * 8;
 #pragma unroll
-      for (int v = 0; v < 5; ++v) cp_async8(d + v * NPT * 8, A.S_prev + o + v * P.N);
-      if (A.f_prev) cp_async8(d + 5 * NPT * 8, A.q_out + o + P.QS);
+      for (int v = 0; v < 5; ++v) cp_async8(d + v * NPT * 8, sp + v * P.N);
+      if (A.f_prev) cp_async8(d + 5 * NPT * 8, (A.q_out + zo + P.QS) + own32);
     }
     cp_async_commit();
     cp_async_wait<1>();                                  // the groups of steps <= s-1 have landed: own node of plane s+3
@@ -685,10 +689,11 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       }
       fsum = fma(R[1], zh[p - k0], fsum);                                      // times h_x h_y after the loop
       // ---------------- epilogue: write R, or the RK3 stage of Eq. 11 ------------------------------
-      const size_t o = (size_t)p * P.nxy + own_off;
+      const long long zo = (long long)p * P.nxy;
       if (!FUSED) {
+        double* ro = (A.out_rhs + zo) + own32;
 #pragma unroll
-        for (int v = 0; v < 5; ++v) A.out_rhs[o + v * P.N] = R[v];
+        for (int v = 0; v < 5; ++v) ro[v * P.N] = R[v];
       } else {
         double dW[5];
         const double dt = scal[0], fprev = scal[1];
@@ -699,16 +704,21 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
           if (v == 1) sp += fprev;
           if (v == 4 && A.f_prev && A.alpha != 0.0) sp = fma(fprev, pv[5 * NPT], sp);
           dW[v] = dt * (A.alpha * sp + A.beta * R[v]);
-          if (A.write_S) A.S_out[o + v * P.N] = R[v];
+        }
+        if (A.write_S) {
+          double* so = (A.S_out + zo) + own32;
+#pragma unroll
+          for (int v = 0; v < 5; ++v) so[v * P.N] = R[v];
         }
         Prim qn; qn.rho = rw[0]; qn.u = uw[0]; qn.v = vw[0]; qn.w = ww[0]; qn.T = Tw[0]; qn.mu = mw[0]; qn.H = 0.0;
         bool store_mu = !LAZY;
         advance_prim<!LAZY>(P, qn, dW);
         if (!PLAIN && gj == 0 && node_wall(P.bc[2])) { wall_node_override(P, P.Twall[0], P.mu_wall[0], qn); store_mu = true; }
         if (!PLAIN && gj == P.ny - 1 && node_wall(P.bc[3])) { wall_node_override(P, P.Twall[1], P.mu_wall[1], qn); store_mu = true; }
-        A.q_out[o] = qn.rho; A.q_out[o + P.QS] = qn.u; A.q_out[o + 2 * P.QS] = qn.v; A.q_out[o + 3 * P.QS] = qn.w;
-        A.q_out[o + 4 * P.QS] = qn.T; A.q_out[o + 6 * P.QS] = qn.H;
-        if (store_mu) A.q_out[o + 5 * P.QS] = qn.mu;
+        double* qo = (A.q_out + zo) + own32;
+        qo[0] = qn.rho; qo[P.QS] = qn.u; qo[2 * P.QS] = qn.v; qo[3 * P.QS] = qn.w;
+        qo[4 * P.QS] = qn.T; qo[6 * P.QS] = qn.H;
+        if (store_mu) qo[5 * P.QS] = qn.mu;
       }
     }
     // ---- second half of the barrier: the staging rows of this plane are complete ----
