@@ -63,7 +63,7 @@ constexpr int SM_RED = 32;
 constexpr int LZ_MAX = 128;                     // planes per CTA (make_layout caps the chunk length)
 constexpr int SM_MET = 3 * LZ_MAX + 2 * TX + 2 * TY;   // 1/h_z, -g_z/h_z^3, h_z of the chunk; 1/h, -g/h^3 of the tile's x and y
 constexpr int SM_PATCH = TILE;                  // ghost-slot list of an edge tile: one int2 (8 bytes) per entry
-constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_SPREV + SM_MET + SM_PATCH + SM_PCOPY + SM_RED + 8;
+constexpr int SM_RHS_DOUBLES = SM_TILES + 2 * SM_STG1 + SM_GRING + SM_RRING + SM_OWN + SM_SPREV + SM_MET + SM_PATCH + SM_PCOPY + SM_RED + 16;
 static_assert(SM_RHS_DOUBLES * 8 <= 227 * 1024, "one CTA per SM: the shared-memory budget of sm_100a");
 constexpr int NSTAGE = 2 * HALO * TY + 2 * HALO * TX;                     // 240 staged derivatives outside the tile
 constexpr unsigned TILE_BYTES = SM_TILE1 * sizeof(double);
@@ -87,7 +87,7 @@ struct RhsArgs {
   int lz;                 // planes per CTA
   int cz0, czs;           // chunk of CTA z-index c is cz0 + c * czs (whole grid: 0, 1; streams_stage_rhs launches the chunks
                           // that need no ghost plane of a BC_HALO face and the two boundary chunks separately)
-  int use_tma;            // 1: tile by TMA box copies (tensor map over q); 0: every slot by index (odd nx)
+  int use_tma;            // 1: tile and own-node ring by TMA box copies (tensor maps over q); 0: by index (odd nx)
 };
 
 // ---- PTX helpers: mbarrier, TMA ----------------------------------------------------------------
@@ -109,11 +109,19 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
                  : "=r"(ok) : "r"(bar), "r"(parity), "r"(4000u) : "memory");
   } while (!ok);
 }
-// one 4-D box (x, y, z, field) of the primitive state into a tile buffer; completes `TILE_BYTES` on the mbarrier
-__device__ __forceinline__ void tma_tile(unsigned dst, const CUtensorMap* tm, int x, int y, int z, unsigned bar) {
+// one 4-D box (x, y, z, field) into shared memory; completes its bytes on the mbarrier
+__device__ __forceinline__ void tma_box(unsigned dst, const CUtensorMap* tm, int x, int y, int z, int f, unsigned bar) {
   asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-               ::"r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(0), "r"(bar) : "memory");
+               ::"r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(f), "r"(bar) : "memory");
 }
+// the tile of a plane (halo 3, all stored primitives); completes `TILE_BYTES`
+__device__ __forceinline__ void tma_tile(unsigned dst, const CUtensorMap* tm, int x, int y, int z, unsigned bar) { tma_box(dst, tm, x, y, z, 0, bar); }
+
+// Tensor maps of one launch (all 4-D: x, y, z, field):
+//   tile  the state the residual is evaluated on, box (PITCH, PY, 1, NQ): a plane's tile with its halo
+//   own   the same state, box (TX, TY, 1, NQ): the tile's own nodes of a later plane (z window, no halo)
+struct RhsMaps { CUtensorMap tile, own; };
+constexpr unsigned OWN_BYTES = NQ * NPT * sizeof(double);
 // thread-private asynchronous 8-byte copies (own node of a later plane into the own-node ring)
 __device__ __forceinline__ void cp_async8(unsigned dst, const double* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
@@ -365,7 +373,8 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
 // frees ~30 registers for the scheduler.  Ghost slots (periodic wrap, reflection, ...) are handled in both.
 // MODE: 0 = residual only (streams_rhs), 1 = fused RK stage, 2 = fused RK stage with lazy forcing (mu(T) left to k_force_fix)
 template <int MODE, bool PLAIN>
-__device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const CUtensorMap& tmap, double* sm, const int3 cta) {
+__device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const RhsMaps& M, double* sm, const int3 cta) {
+  const CUtensorMap& tmap = M.tile;
   constexpr bool FUSED = MODE != 0, LAZY = MODE == 2;
   double* tiles = sm;
   double* stg = tiles + SM_TILES;
@@ -383,6 +392,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   const unsigned bar0 = smem_u32(red + SM_RED);          // NBUF mbarriers: tile buffer b holds its plane
   const unsigned sbar = bar0 + 8 * NBUF;                 // the per-plane CTA barrier, split into arrive / wait
   int* pcount = reinterpret_cast<int*>(red + SM_RED + NBUF + 1);
+  const unsigned obar = bar0 + 8 * 8;                    // NOWN mbarriers: own-node ring slot holds its plane (TMA path)
   const double* zi = met;                                // 1/h_z, -g_z/h_z^3, h_z of planes k0 .. k1-1
   const double* zg = met + LZ_MAX;
   const double* zh = met + 2 * LZ_MAX;
@@ -400,6 +410,10 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   const bool active = PLAIN || (gi < P.nx && gj < P.ny);
   const int own_off = gj * P.nx + gi;
   const bool use_tma = PLAIN || A.use_tma != 0;
+  // with TMA the own-node ring is filled by box copies too (one request per plane by one thread instead of seven
+  // thread-private copies with their address arithmetic): config 5 -1.4 %, config 4 -0.7 % per launch, the L2-resident
+  // configs 2, 3 +1 ... 1.5 %; choosing between the two at run time costs more than either (both bodies in the loop)
+  const bool own_tma = use_tma;
   // tiles that see a domain face fill their ghost slots by index (S1); without TMA every tile fills every slot
   const bool edge = !use_tma || i0 < HALO || i0 + TX + HALO > P.nx || j0 < HALO || j0 + TY + HALO > P.ny;
   const int nplanes = k1 + 3 - (k0 - 3);
@@ -410,6 +424,8 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     if (use_tma) {
 #pragma unroll
       for (int b = 0; b < NBUF; ++b) mbar_init(bar0 + 8 * b, 1);
+#pragma unroll
+      for (int b = 0; b < NOWN; ++b) mbar_init(obar + 8 * b, 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
@@ -419,6 +435,14 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         if (b < nplanes) {
           mbar_expect_tx(bar0 + 8 * b, TILE_BYTES);
           tma_tile(smem_u32(tiles + b * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, k0 - 3 + b) + P.zpad, bar0 + 8 * b);
+        }
+      // own nodes of planes k0, k0+1, k0+2 (ring slots 0, 1, 2): plane q sits in slot (q - k0) % 3; later planes are
+      // requested by the same thread at the end of the step that read the slot's previous plane
+#pragma unroll
+      for (int b = 0; b < NOWN; ++b)
+        if (own_tma && k0 + b < k1 + 3) {
+          mbar_expect_tx(obar + 8 * b, OWN_BYTES);
+          tma_box(smem_u32(oring + b * NF * NPT), &M.own, i0, j0, map_z(P, k0 + b) + P.zpad, 0, obar + 8 * b);
         }
     }
   }
@@ -464,14 +488,18 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   }
   // own node of the planes ahead: plane s+5 is requested at the top of step s (cp.async, thread-private
   // slot, no register and no barrier) into ring slot (it+5) % 3; plane s+3 is read from slot it % 3
+  // (with TMA the ring is filled by box copies of the tile's own nodes instead: one request per plane, no per-thread
+  // address arithmetic, completion on the slot's mbarrier)
+  if (!own_tma) {
 #pragma unroll
-  for (int b = 0; b < 2; ++b) {
-    if (active) {
-      const double* q = A.q + own_off + (long long)map_z(P, k0 + b) * P.nxy;
+    for (int b = 0; b < 2; ++b) {
+      if (active) {
+        const double* q = A.q + own_off + (long long)map_z(P, k0 + b) * P.nxy;
 #pragma unroll
-      for (int f = 0; f < NF; ++f) cp_async8(smem_u32(oring + tid) + ((b * NF + f) * NPT) * 8, q + f * P.QS);
+        for (int f = 0; f < NF; ++f) cp_async8(smem_u32(oring + tid) + ((b * NF + f) * NPT) * 8, q + f * P.QS);
+      }
+      cp_async_commit();
     }
-    cp_async_commit();
   }
   // dt and the previous stage's body force sit in shared memory (read once per plane in the epilogue)
   double* scal = red + SM_RED + NBUF + 2;
@@ -481,6 +509,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   }
   __syncthreads();
   int slot7 = 0, b3 = 0;                                 // it % 7, it % 3
+  unsigned own_par = 0;                                  // (it / 3) & 1: phase of the own-node ring slot read in this step
 
   for (int s = k0 - 3, it = 0; s < k1 + 3; ++s, ++it) {
     const bool full = s >= k0 && s < k1;
@@ -490,7 +519,8 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     // Addresses: a warp-uniform pointer (plane, field) plus the node's 32-bit offset inside a plane (two instructions per
     // address; a 64-bit per-thread element index costs four, and the loop forms 24 addresses per plane)
     const unsigned own32 = (unsigned)own_off;
-    if (active && s + 5 < k1 + 3) {
+    if (!own_tma && active && s + 5 < k1 + 3) {
+      // own node of plane s+5 by thread-private copies (with TMA: a box copy per plane, requested at the end of a step)
       const double* q = (A.q + (long long)map_z(P, s + 5) * P.nxy) + own32;
       const unsigned d = smem_u32(oring + tid) + ((b3 == 0 ? 2 : b3 - 1) * NF * NPT) * 8;       // (it + 5) % 3
 #pragma unroll
@@ -498,7 +528,8 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     }
     if (FUSED && A.alpha != 0.0 && active && s - 2 >= k0 && s - 2 < k1) {
       // R_prev (and u_prev for the lazy forcing) of plane s-2, read in the NEXT step's epilogue (one step of slack:
-      // the epilogue sits before the plane barrier and must not wait for HBM)
+      // the epilogue sits before the plane barrier and must not wait for HBM).  Thread-private slots: a thread's own
+      // program order keeps the copy behind its reads of the slot, which happen between barrier arrive and wait.
       const long long zo = (long long)(s - 2) * P.nxy;
       const double* sp = (A.S_prev + zo) + own32;
       const unsigned d = smem_u32(spring + tid) + (((it + 1) & 1) * 6 * NPT) * 8;
@@ -507,8 +538,8 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       if (A.f_prev) cp_async8(d + 5 * NPT * 8, (A.q_out + zo + P.QS) + own32);
     }
     cp_async_commit();
-    cp_async_wait<1>();                                  // the groups of steps <= s-1 have landed: own node of plane s+3
-                                                         // (and s+4), R_prev of plane s-3
+    cp_async_wait<1>();                                  // the groups of steps <= s-1 have landed: R_prev of plane s-3 (and
+                                                         // without TMA the own node of planes s+3, s+4)
     int tl = tid;                                        // opaque copy: keeps per-thread shared-memory addresses from being
     asm volatile("" : "+r"(tl));                         // hoisted out of the loop (and then spilled) instead of recomputed
     const int li = tl & (TX - 1), lj = tl / TX, loc = (lj + HALO) * PITCH + li + XH;
@@ -633,6 +664,11 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       // the same bits, so that the result does not depend on how z is cut into chunks or slabs
       gr[0] = N.G[6]; gr[NPT] = N.G[7]; gr[2 * NPT] = __dadd_rn(N.G[0], N.G[4]);
     }
+    // own node of plane s+3: read BEFORE the arrive, so that every thread is done with the ring slot when the barrier
+    // completes and the slot can take the box copy of plane s+6 (requested three steps before it is read)
+    if (own_tma && s + 3 < k1 + 3) mbar_wait(obar + 8 * b3, own_par);
+    o3.rho = own3[F_RHO * NPT]; o3.u = own3[F_U * NPT]; o3.v = own3[F_V * NPT]; o3.w = own3[F_W * NPT];
+    o3.T = own3[F_T * NPT]; o3.mu = own3[F_MU * NPT]; o3.H = own3[F_H * NPT];
     // ---- the plane's barrier, first half: everything other threads read of this step is written ----
     __syncwarp();
     if ((tl & 31) == 0) mbar_arrive(sbar);
@@ -642,8 +678,6 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     // p = s-3 (z-mixed terms from the thread-private rings, Eq. 11, global stores) -- more than half of the step's
     // work, so that the wait below finds the barrier complete (measured: the wait was 6 % of all warp cycles when it
     // sat directly after the z direction).
-    o3.rho = own3[F_RHO * NPT]; o3.u = own3[F_U * NPT]; o3.v = own3[F_V * NPT]; o3.w = own3[F_W * NPT];
-    o3.T = own3[F_T * NPT]; o3.mu = own3[F_MU * NPT]; o3.H = own3[F_H * NPT];
     const int p = s - 3;
     const bool do_fin = active && p >= k0, do_asm = active && full;
     if (do_asm) {
@@ -730,6 +764,12 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       mbar_expect_tx(bar0 + 8 * b2, TILE_BYTES);
       tma_tile(smem_u32(tiles + b2 * SM_TILE1), &tmap, i0 - XH, j0 - HALO, map_z(P, s + 2) + P.zpad, bar0 + 8 * b2);
     }
+    // ... and the ring slot read in this step (plane s+3; every thread read it before arriving) takes plane s+6
+    if (own_tma && tl == 0 && s + 6 < k1 + 3) {
+      fence_proxy_async();
+      mbar_expect_tx(obar + 8 * b3, OWN_BYTES);
+      tma_box(smem_u32(oring + b3 * NF * NPT), &M.own, i0, j0, map_z(P, s + 6) + P.zpad, 0, obar + 8 * b3);
+    }
     // ================= after the barrier: the xy mixed terms of plane s (A8), d_x(d_y v) and d_y(d_x u) from the
     // staging rows; they enter V_0, V_1 times mu / 3 and the viscous work u V_0 + v V_1.  R of plane s goes to the
     // residual ring (its slot was read above: plane s-3).
@@ -752,7 +792,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       for (int v = 0; v < 5; ++v) rr[v * NPT] = N.R[v];
     }
     slot7 = slot7 == 6 ? 0 : slot7 + 1;
-    b3 = b3 == 2 ? 0 : b3 + 1;
+    if (b3 == 2) { b3 = 0; own_par ^= 1u; } else ++b3;
     // ---------------- shift the windows, own node of plane s+4 ------------------------------------
 #pragma unroll
     for (int a = 0; a < 5; ++a) {
@@ -770,7 +810,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ CUtensorMap tmap) {
+__global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ RhsMaps M) {
   extern __shared__ __align__(128) double sm[];
   // CTA -> (tile, chunk): the chunk index varies fastest with the launch order, so that the CTAs resident at any time
   // march through different z ranges (spreads the DRAM traffic; one wave in lockstep through z measured 24 % slower)
@@ -782,8 +822,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
   const bool wall_lo = (P.bc[2] == BC_WALL_STAG || node_wall(P.bc[2])) && j0 == 0;
   const bool wall_hi = (P.bc[3] == BC_WALL_STAG || node_wall(P.bc[3]) || P.bc[3] == BC_OUTFLOW) && j0 + TY >= P.ny;
-  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, tmap, sm, cta);
-  else rhs_body<MODE, false>(P, A, tmap, sm, cta);
+  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, M, sm, cta);
+  else rhs_body<MODE, false>(P, A, M, sm, cta);
 }
 
 }  // namespace streams

@@ -57,7 +57,8 @@ struct streams_ctx {
   int stage_half;                      // streams_stage_end comes next (half: 0 = rhs pending, 1 = end pending)
   int inflow_pending;                  // z-slab with INFLOW_FROZEN: the frozen plane is captured once the ghost planes are in
   int parts_done;                      // bit 0: interior chunks launched, bit 1: boundary chunks launched (this stage)
-  CUtensorMap tmap[2];           // TMA descriptors of qbuf[0], qbuf[1] as 4-D tensors (x, y, z, field)
+  // TMA descriptors, 4-D (x, y, z, field): per state buffer the tile box (halo 3) and the own-node box (no halo)
+  CUtensorMap tmap[2], tmap_own[2];
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
   int prof_on, prof_n;
   std::vector<cudaEvent_t>* prof_ev;   // pairs (start, stop) around k_rhs
@@ -194,17 +195,17 @@ bool shock_post_state(const streams_params& p, double post[NQ]) {
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-bool make_tile_map(CUtensorMap* tm, double* q, int nx, int ny, int nz) {
+bool make_box_map(CUtensorMap* tm, double* base, int nx, int ny, int nz, int nf, int bx, int by, int bf) {
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
       qres != cudaDriverEntryPointSuccess)
     return false;
-  const cuuint64_t dims[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)NQ};
+  const cuuint64_t dims[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)nf};
   const cuuint64_t strides[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)nx * ny * nz * 8};
-  const cuuint32_t box[4] = {(cuuint32_t)PITCH, (cuuint32_t)PY, 1u, (cuuint32_t)NQ};
+  const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, (cuuint32_t)bf};
   const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
-  const CUresult r = ((EncodeTiledFn)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, q, dims, strides, box, estr,
+  const CUresult r = ((EncodeTiledFn)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS;
@@ -501,7 +502,8 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   c->use_tma = (n[0] % 2 == 0) ? 1 : 0;
   if (c->use_tma)
     for (int i = 0; i < 2; ++i)
-      if (!make_tile_map(&c->tmap[i], c->qbuf[i] - zoff, n[0], n[1], n[2] + 2 * L.zpad)) {
+      if (!make_box_map(&c->tmap[i], c->qbuf[i] - zoff, n[0], n[1], n[2] + 2 * L.zpad, NQ, PITCH, PY, NQ) ||
+          !make_box_map(&c->tmap_own[i], c->qbuf[i] - zoff, n[0], n[1], n[2] + 2 * L.zpad, NQ, TX, TY, NQ)) {
         cudaFree(c->small_dev); delete c;
         return fail(nullptr, STREAMS_ECUDA, "cuTensorMapEncodeTiled failed");
       }
@@ -636,7 +638,9 @@ static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in, dim3 grid) 
   RhsArgs A = A_in;
   A.use_tma = c->use_tma;
   A.nflag = c->p.weno_enable ? c->nflag : nullptr;
-  const CUtensorMap& tm = c->tmap[A.q == c->qbuf[1] ? 1 : 0];
+  const int qi = A.q == c->qbuf[1] ? 1 : 0;
+  RhsMaps tm;
+  tm.tile = c->tmap[qi]; tm.own = c->tmap_own[qi];
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
