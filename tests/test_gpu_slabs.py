@@ -341,3 +341,31 @@ def test_config5_size_two_slabs_one_step_bitwise(env):
     assert abs(d[0].mass + d[1].mass - d[2].mass) <= 1e-12 * d[2].mass
     for c in ctxs + [one]:
         c.close()
+
+
+def test_non_periodic_z_ends_keep_their_boundary(env):
+    """z faces that are physical boundaries (zeroth-order extrapolation) stay with the first and the last slab; only the
+    internal faces become BC_HALO (one-sided halos): three slabs are bitwise the undivided run."""
+    torch, binding, slab, ob = env
+    p = W.default_params(Rgas=1 / 1.4, mu_ref=5e-3)
+    p["bc"] = [0, 0, 0, 0, W.BC_EXTRAP, W.BC_EXTRAP]
+    wl = W.random_periodic(40, 20, 36, params=p)
+    w0 = wl.state()
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(w0).cuda())
+    one.step(3)
+    ref = one.get_state().cpu().numpy()
+    ctxs, specs, _ = make_slabs(env, wl, 3)
+    assert [sp.params["bc"][4:] for sp in specs] == [[W.BC_EXTRAP, 8], [8, 8], [8, W.BC_EXTRAP]]
+    grp = slab.SlabGroup(ctxs, 3, periodic=False, reducer=HostReducer(torch), forcing=False, cfl_dt=True)
+    grp.step(3)
+    got = gather(ctxs)
+    assert np.array_equal(got, ref), np.abs(got - ref).max()
+    assert grp.messages_sent == 3 * 3 * 4
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    o.set_state(w0)
+    o.step(3)
+    assert l2(got, o.get_state()) < STEP_TOL
+    for c in ctxs + [one]:
+        c.close()
+    o.close()
