@@ -575,12 +575,6 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       N.Va[0] = N.Va[1] = N.Va[2] = 0.0; N.LT = 0.0; N.heat = 0.0;
     }
     if (use_tma) mbar_wait(bar0 + 8 * buf, phase);
-    if (edge && it + 1 < nplanes) {
-      // ghost slots of the NEXT plane's tile: written before this step's barrier, read after it
-      const int b1 = buf ^ 1;
-      if (use_tma && tl < npatch) mbar_wait(bar0 + 8 * b1, (unsigned)((it + 1) >> 1) & 1u);
-      patch_tile(*sP, A.q, plist, npatch, map_z(P, s + 1), tiles + b1 * SM_TILE1, tl);
-    }
     double* sgY = stg + (it & 1) * SM_STG1;
     double* sgX = sgY + SM_STGY;
     // staged derivative outside the tile: threads [0,48) D_y v on the x-halo columns, [48,240) D_x u on the y-halo rows
@@ -663,6 +657,14 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       // no FMA contraction here: a plane next to a chunk is a ghost plane of that chunk (branch above) and must give
       // the same bits, so that the result does not depend on how z is cut into chunks or slabs
       gr[0] = N.G[6]; gr[NPT] = N.G[7]; gr[2 * NPT] = __dadd_rn(N.G[0], N.G[4]);
+    }
+    if (edge && it + 1 < nplanes) {
+      // ghost slots of the NEXT plane's tile: written before this step's barrier, read after it.  Done here, after the
+      // in-plane work, because that tile was requested at the end of the previous step: waiting for it at the top of the
+      // step exposed the whole TMA latency on the patching warps, and through the barrier on everybody
+      const int b1 = buf ^ 1;
+      if (use_tma && tl < npatch) mbar_wait(bar0 + 8 * b1, (unsigned)((it + 1) >> 1) & 1u);
+      patch_tile(*sP, A.q, plist, npatch, map_z(P, s + 1), tiles + b1 * SM_TILE1, tl);
     }
     // own node of plane s+3: read BEFORE the arrive, so that every thread is done with the ring slot when the barrier
     // completes and the slot can take the box copy of plane s+6 (requested three steps before it is read)
