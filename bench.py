@@ -42,14 +42,14 @@ def make_workload(cfg: int, zcopies: int = 1):
         return W.config5_channel_big(zcopies=zcopies)
     if cfg == 3:
         return W.config3_channel(zcopies=zcopies)
+    if cfg == 4:
+        return W.config4_sbli(zcopies=zcopies)
     if zcopies != 1:
-        raise SystemExit("--decomp slab: configs 3 and 5 (channel, periodic z, central scheme) only")
+        raise SystemExit("--decomp slab with more than one slab: configs 3, 4 and 5 (their z is periodic and homogeneous)")
     if cfg == 1:
         return W.config1_tgv()
     if cfg == 2:
         return W.config2_isotropic()
-    if cfg == 4:
-        return W.config4_sbli()
     if cfg == 6:                       # the paper-literal channel numerics (4th order, Sutherland, erf grid) at config-3 size
         return W.config6_channel_paper(256, 128, 128)
     raise SystemExit(f"unknown config {cfg}")
@@ -198,7 +198,7 @@ def run_ours(args, rank, world, local_rank):
 
     decomp = args.decomp
     if decomp == "auto":
-        decomp = "slab" if world > 1 and args.config in (3, 5) else ("replicas" if world > 1 else "single")
+        decomp = "slab" if world > 1 and args.config in (3, 4, 5) else ("replicas" if world > 1 else "single")
     grp = None
     slab_error = None
     if decomp == "slab":
@@ -215,7 +215,8 @@ def run_ours(args, rank, world, local_rank):
             w0 = upload_state(torch, glob, dev, k0=sp.k0, k1=sp.k1)
             s.set_state(w0)
             grp = slab_mod.SlabGroup([s], world, rank=rank, periodic=True, dist=dist, forcing=bool(glob.params["forcing"]),
-                                     cfl_dt=not glob.params["dt_fixed"] > 0, overlap=not args.no_overlap)
+                                     cfl_dt=not glob.params["dt_fixed"] > 0, overlap=not args.no_overlap,
+                                     weno=bool(glob.params["weno_enable"]))
             grp.step(1)                        # sets up the point-to-point communicators; part of the warm-up
             torch.cuda.synchronize(dev)
         except Exception as e:                 # noqa: BLE001 -- reported, never silent
@@ -398,7 +399,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--decomp", default="auto", choices=["auto", "single", "replicas", "slab"],
-                    help="auto: 1 GPU -> single context; N GPUs -> z-slabs (configs 3, 5), else replicas")
+                    help="auto: 1 GPU -> single context; N GPUs -> z-slabs (configs 3, 4, 5), else replicas")
     ap.add_argument("--no-overlap", action="store_true", help="slab mode: swap the halos before the whole stage kernel")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

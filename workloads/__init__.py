@@ -307,8 +307,10 @@ def config7_boundary_layer(nx=256, ny=64, nz=32, seed=1007, steps=20, Lx=24.0, L
     return config4_sbli(nx, ny, nz, seed, steps, Lx, Ly, Lz, M=2.0, shock=False, name="boundary_layer")
 
 
-def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0, Lz=4.0, M=2.28, shock=True, name="sbli") -> Workload:
+def config4_sbli(nx=1024, ny=256, nz=128, seed=1004, steps=100, Lx=48.0, Ly=8.0, Lz=4.0, M=2.28, shock=True, name="sbli", zcopies=1) -> Workload:
+    """zcopies > 1: a span zcopies times as wide (nz and L_z scaled together): the weak-scaling input of the z-slab mode."""
     gamma, Pr = 1.4, 0.72
+    nz, Lz = nz * zcopies, Lz * zcopies
     x = Lx * np.arange(nx) / (nx - 1.0)
     z = Lz * np.arange(nz) / nz
     y = sinh_nodes(ny, Ly)
