@@ -297,26 +297,31 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
   const double c2 = P.gm1 * (Hb - 0.5 * q2), cb = sqrt(c2), icb = 1.0 / cb;
   const double b1 = P.gm1 / c2, b2 = 0.5 * q2 * b1;
   const double un = ub[D];
-  // steps 3-4: characteristic variables/fluxes at the six nodes, local LF speeds
+  // steps 3-4: characteristic variables/fluxes at the six nodes, local LF speeds.  With w = (rho, rho u, rho H - p) and
+  // f = vn w + p (e_{1+D} + vn e_5) the projections l_s . w and l_s . f collapse to a few operations per node:
+  //   a = rho (b2 + b1 (H - ub.u)) - b1 p,   d = rho (un - vn) / cb
+  //   l_1,5 . w = (a +- d) / 2,  l_2 . w = rho - a,  l_3,4 . w = rho (u_T - ub_T)
+  //   l_s . f = vn (l_s . w) + p (l_s[1+D] + vn l_s[5]):  e = b1 (vn - un) p, h = p / cb:  (e -+ h)/2, -e, 0, 0
+  // (the same left eigenvectors as SURVEY S6, multiplied out; equal to the matrix-vector products up to rounding)
   double wc[6][5], fc[6][5], al[5] = {0, 0, 0, 0, 0};
 #pragma unroll
   for (int n = 0; n < 6; ++n) {
     const double vn = vel[n][D];
-    const double wv[5] = {rho[n], rho[n] * vel[n][0], rho[n] * vel[n][1], rho[n] * vel[n][2], rho[n] * Hh[n] - pp[n]};
-    double fv[5] = {rho[n] * vn, wv[1] * vn, wv[2] * vn, wv[3] * vn, rho[n] * vn * Hh[n]};
-    fv[1 + D] += pp[n];
-    const double mw = ub[0] * wv[1] + ub[1] * wv[2] + ub[2] * wv[3];
-    const double mf = ub[0] * fv[1] + ub[1] * fv[2] + ub[2] * fv[3];
-    wc[n][0] = 0.5 * ((b2 + un * icb) * wv[0] - b1 * mw - wv[1 + D] * icb + b1 * wv[4]);
-    fc[n][0] = 0.5 * ((b2 + un * icb) * fv[0] - b1 * mf - fv[1 + D] * icb + b1 * fv[4]);
-    wc[n][1] = (1.0 - b2) * wv[0] + b1 * mw - b1 * wv[4];
-    fc[n][1] = (1.0 - b2) * fv[0] + b1 * mf - b1 * fv[4];
-    wc[n][2] = -ub[T1] * wv[0] + wv[1 + T1];
-    fc[n][2] = -ub[T1] * fv[0] + fv[1 + T1];
-    wc[n][3] = -ub[T2] * wv[0] + wv[1 + T2];
-    fc[n][3] = -ub[T2] * fv[0] + fv[1 + T2];
-    wc[n][4] = 0.5 * ((b2 - un * icb) * wv[0] - b1 * mw + wv[1 + D] * icb + b1 * wv[4]);
-    fc[n][4] = 0.5 * ((b2 - un * icb) * fv[0] - b1 * mf + fv[1 + D] * icb + b1 * fv[4]);
+    const double m = ub[0] * vel[n][0] + ub[1] * vel[n][1] + ub[2] * vel[n][2];
+    const double g = b2 + b1 * (Hh[n] - m);
+    const double a = rho[n] * g - b1 * pp[n];
+    const double d = icb * (rho[n] * (un - vn));
+    wc[n][0] = 0.5 * (a + d);
+    wc[n][1] = rho[n] - a;
+    wc[n][2] = rho[n] * (vel[n][T1] - ub[T1]);
+    wc[n][3] = rho[n] * (vel[n][T2] - ub[T2]);
+    wc[n][4] = 0.5 * (a - d);
+    const double e = b1 * ((vn - un) * pp[n]), h = icb * pp[n];
+    fc[n][0] = vn * wc[n][0] + 0.5 * (e - h);
+    fc[n][1] = vn * wc[n][1] - e;
+    fc[n][2] = vn * wc[n][2];
+    fc[n][3] = vn * wc[n][3];
+    fc[n][4] = vn * wc[n][4] + 0.5 * (e + h);
     al[0] = fmax(al[0], fabs(vn - cs[n]));
     al[1] = fmax(al[1], fabs(vn));
     al[4] = fmax(al[4], fabs(vn + cs[n]));
