@@ -397,7 +397,7 @@ __device__ __forceinline__ void dF_below(const DevP& P, const double* __restrict
   for (int v = 0; v < 5; ++v) dF[v] = in[o + v * P.N];
 }
 
-// one thread per listed node: R += dR, and (if q_new) the node of the already advanced state takes the
+// one thread per listed node: R += dR (if R), and (if q_new) the node of the already advanced state takes the
 // conservative increment dt beta dR  (Eq. 11 is linear in R)
 __global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ list,
                                                    const unsigned char* __restrict__ lmask, const DevScal* __restrict__ sc,
@@ -441,8 +441,10 @@ __global__ void __launch_bounds__(RT) k_weno_apply(const __grid_constant__ DevP 
 #pragma unroll
         for (int v = 0; v < 5; ++v) dR[v] -= ih * dFbuf[(size_t)10 * P.N + o + v * P.N]; }
     }
+    if (R) {                                             // NULL in the last RK stage: its R is never read
 #pragma unroll
-    for (int v = 0; v < 5; ++v) R[o + v * P.N] += dR[v];
+      for (int v = 0; v < 5; ++v) R[o + v * P.N] += dR[v];
+    }
     if (q_new) {
       const bool wall = (j == 0 && node_wall(P.bc[2])) || (j == P.ny - 1 && node_wall(P.bc[3]));
       if (wall) {

@@ -761,7 +761,8 @@ static int do_stage_rhs(streams_ctx* c, int l, int part, bool single) {
     if (last && c->p.weno_enable && (rc = run_flag_pack(c))) return rc;
   } else {
     // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
-    A.q_out = c->qbuf[c->cur ^ 1]; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = 1;   // k_weno_apply may still add to S
+    // R of the last stage is never read (alpha_0 = 0): neither this kernel nor k_weno_apply stores it
+    A.q_out = c->qbuf[c->cur ^ 1]; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = l < 2 ? 1 : 0;
     if (any && (rc = launch_rhs(c, 1, A, grid))) return rc;
     if (last && c->p.weno_enable && (rc = run_flag_pack(c))) return rc;
   }
@@ -795,7 +796,7 @@ static int do_stage_end(streams_ctx* c, int l, bool single) {
     LAUNCH_CHECK("k_update");
     c->scur ^= 1;
   } else {
-    if (c->p.weno_enable && (rc = run_weno(c, w, c->S[0], c->qbuf[c->cur ^ 1], RK_BETA[l]))) return rc;
+    if (c->p.weno_enable && (rc = run_weno(c, w, l < 2 ? c->S[0] : nullptr, c->qbuf[c->cur ^ 1], RK_BETA[l]))) return rc;
     c->cur ^= 1;
   }
   if (l == 2) {
