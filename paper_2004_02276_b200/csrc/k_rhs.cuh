@@ -757,6 +757,15 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         if (store_mu) qo[5 * P.QS] = qn.mu;
       }
     }
+    // ---------------- shift the windows (own node of plane s+3 enters) BEFORE the wait: 70 register moves that need no
+    // other thread, done while the barrier completes.  After the shift the plane's own node sits in slot 2.
+#pragma unroll
+    for (int a = 0; a < 5; ++a) {
+      rw[a] = rw[a + 1]; uw[a] = uw[a + 1]; vw[a] = vw[a + 1]; ww[a] = ww[a + 1]; Tw[a] = Tw[a + 1]; mw[a] = mw[a + 1]; Hw[a] = Hw[a + 1];
+    }
+    if (active && s + 3 < k1 + 3) {
+      rw[5] = o3.rho; uw[5] = o3.u; vw[5] = o3.v; ww[5] = o3.w; Tw[5] = o3.T; mw[5] = o3.mu; Hw[5] = o3.H;
+    }
     // ---- second half of the barrier: the staging rows of this plane are complete ----
     mbar_wait(sbar, (unsigned)(it & 1));
     // every thread is past its reads of this plane's tile: the buffer takes plane s+2
@@ -784,10 +793,10 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         double myx = P.c.a[0] * (sgX[sx + TX] - sgX[sx - TX]);
         myx = fma(P.c.a[1], sgX[sx + 2 * TX] - sgX[sx - 2 * TX], myx);
         myx = fma(P.c.a[2], sgX[sx + 3 * TX] - sgX[sx - 3 * TX], myx);
-        const double m3 = mw[3] * (xi[li] * yi[lj] * (1.0 / 3.0));
+        const double m3 = mw[2] * (xi[li] * yi[lj] * (1.0 / 3.0));        // slot 2: the windows are already shifted
         const double v0 = m3 * mxy, v1 = m3 * myx;
         N.R[1] += v0; N.R[2] += v1;
-        N.R[4] += fma(uw[3], v0, vw[3] * v1);
+        N.R[4] += fma(uw[2], v0, vw[2] * v1);
       }
       double* rr = rring + b3 * 5 * NPT + tl;
 #pragma unroll
@@ -795,14 +804,6 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     }
     slot7 = slot7 == 6 ? 0 : slot7 + 1;
     if (b3 == 2) { b3 = 0; own_par ^= 1u; } else ++b3;
-    // ---------------- shift the windows, own node of plane s+4 ------------------------------------
-#pragma unroll
-    for (int a = 0; a < 5; ++a) {
-      rw[a] = rw[a + 1]; uw[a] = uw[a + 1]; vw[a] = vw[a + 1]; ww[a] = ww[a + 1]; Tw[a] = Tw[a + 1]; mw[a] = mw[a + 1]; Hw[a] = Hw[a + 1];
-    }
-    if (active && s + 3 < k1 + 3) {
-      rw[5] = o3.rho; uw[5] = o3.u; vw[5] = o3.v; ww[5] = o3.w; Tw[5] = o3.T; mw[5] = o3.mu; Hw[5] = o3.H;
-    }
   }
   if (A.partial) {
     const double hxy = active ? P.hh[0][gi] * P.hh[1][gj] : 0.0;
