@@ -208,15 +208,18 @@ def test_staged_calls_enforce_their_order(env):
         binding.Streams(wl.grid, wl.x, wl.y, wl.z, p)
 
 
-def test_nccl_self_exchange_world_size_one(env):
+@pytest.mark.parametrize("case", ["channel_forcing", "sbli_weno"])
+def test_nccl_self_exchange_world_size_one(env, case):
     """The torch.distributed (NCCL) path of SlabGroup on one GPU: a single periodic slab whose two faces are BC_HALO
     sends its messages to itself through ncclSend/ncclRecv and all-reduces its partial reductions (world size 1: no rank
-    waits on another rank's kernels).  Result: bitwise the periodic single-context run."""
+    waits on another rank's kernels).  Result: bitwise the periodic single-context run.  `sbli_weno` also moves the
+    node-flag words of the hybrid switch (int32 messages) and captures the frozen inflow after the first swap."""
     torch, binding, slab, ob = env
     import torch.distributed as dist
     if not dist.is_nccl_available():
         pytest.skip("NCCL backend not available")
-    wl = W.config3_channel(48, 24, 24)
+    wl = W.config3_channel(48, 24, 24) if case == "channel_forcing" else W.config4_sbli(64, 40, 16)
+    weno = bool(wl.params["weno_enable"])
     w0 = wl.state()
     one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
     one.set_state(torch.from_numpy(w0).cuda())
@@ -233,11 +236,11 @@ def test_nccl_self_exchange_world_size_one(env):
         assert sp.params["bc"][4] == 8 and sp.params["bc"][5] == 8 and len(sp.z) == wl.grid["nz"] + 6
         c = binding.Streams(sp.grid, wl.x, wl.y, sp.z, sp.params)
         c.set_state(torch.from_numpy(w0).cuda())
-        grp = slab.SlabGroup([c], 1, rank=0, periodic=True, dist=dist, forcing=True)
+        grp = slab.SlabGroup([c], 1, rank=0, periodic=True, dist=dist, forcing=bool(wl.params["forcing"]), weno=weno)
         grp.step(2)
         got = c.get_state().cpu().numpy()
         assert np.array_equal(got, ref), np.abs(got - ref).max()
-        assert grp.messages_sent == 2 * 3 * 2
+        assert grp.messages_sent == 2 * 3 * 2 * (2 if weno else 1)
         c.close()
     finally:
         if created:
