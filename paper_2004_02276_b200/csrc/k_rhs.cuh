@@ -81,8 +81,9 @@ struct RhsArgs {
                           // u_prev = the velocity still sitting in q_out (the previous stage's input state)
   double alpha, beta;
   int write_S;            // FUSED: 0 in the last stage (alpha of the next stage is 0: R is never read)
-  unsigned char* nflag;   // hybrid switch on: node flags theta > theta_th of Eq. 8 (a3), a by-product of the velocity
-                          // gradients; [N] bytes, NULL when the WENO switch is off
+  unsigned int* fbits;    // hybrid switch on: node flags theta > theta_th of Eq. 8 (a3), a by-product of the velocity
+                          // gradients, one BIT per node: word [k * ny + j][i / 32] = the ballot of a tile row (= one warp);
+                          // NULL when the WENO switch is off
   double* partial;        // per-CTA partial sums of R_rhou * vol (forcing), may be NULL
   int lz;                 // planes per CTA
   int cz0, czs;           // chunk of CTA z-index c is cz0 + c * czs (whole grid: 0, 1; streams_stage_rhs launches the chunks
@@ -372,7 +373,7 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
 // viscous terms on: every such test folds at compile time and no out-of-line call remains in the plane loop, which
 // frees ~30 registers for the scheduler.  Ghost slots (periodic wrap, reflection, ...) are handled in both.
 // MODE: 0 = residual only (streams_rhs), 1 = fused RK stage, 2 = fused RK stage with lazy forcing (mu(T) left to k_force_fix)
-template <int MODE, bool PLAIN>
+template <int MODE, bool PLAIN, bool WENO>
 __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const RhsMaps& M, double* sm, const int3 cta) {
   const CUtensorMap& tmap = M.tile;
   constexpr bool FUSED = MODE != 0, LAZY = MODE == 2;
@@ -682,21 +683,27 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
     // sat directly after the z direction).
     const int p = s - 3;
     const bool do_fin = active && p >= k0, do_asm = active && full;
+    bool flagged = false;
     if (do_asm) {
       zdir();
-      if (A.nflag) {
+      if (WENO) {
         // S4 / Eq. 8: same expression, same order as k_sensor (the flags must agree bit for bit)
         const double* G = N.G;
         const double div = G[0] + G[4] + G[8];
         const double ox = G[7] - G[5], oy = G[2] - G[6], oz = G[3] - G[1];
         const double th = fmax(-div / sqrt(div * div + (ox * ox + oy * oy + oz * oz) + P.th_eps), 0.0);
-        A.nflag[(size_t)s * P.nxy + own_off] = th > P.th_thr ? 1 : 0;
+        flagged = th > P.th_thr;
       }
       if (PLAIN || P.viscous) {
         Nb c;
         c.rho = rw[3]; c.u = uw[3]; c.v = vw[3]; c.w = ww[3]; c.T = Tw[3]; c.mu = mw[3]; c.H = Hw[3];
         visc_assemble(P, c, N);                          // N.R is final up to the xy mixed terms (added after the wait)
       }
+    }
+    if (WENO && full) {
+      // a tile row is one warp and starts at a multiple of 32: its ballot IS the flag word (0 for nodes beyond the grid)
+      const unsigned bits = __ballot_sync(0xffffffffu, flagged);
+      if ((tl & 31) == 0 && gj < P.ny) A.fbits[((long long)s * P.ny + gj) * ((P.nx + 31) >> 5) + (i0 >> 5)] = bits;
     }
     if (do_fin) {
       double R[5];
@@ -812,7 +819,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   }
 }
 
-template <int MODE>
+// WENO: the hybrid switch is on (the kernel also writes the node flag words); a template parameter, so that the flag code
+// does not exist in the launches of the central-only configs (it cost them 1.7 % as a run-time branch)
+template <int MODE, bool WENO>
 __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ RhsMaps M) {
   extern __shared__ __align__(128) double sm[];
   // CTA -> (tile, chunk): the chunk index varies fastest with the launch order, so that the CTAs resident at any time
@@ -825,8 +834,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
   const bool wall_lo = (P.bc[2] == BC_WALL_STAG || node_wall(P.bc[2])) && j0 == 0;
   const bool wall_hi = (P.bc[3] == BC_WALL_STAG || node_wall(P.bc[3]) || P.bc[3] == BC_OUTFLOW) && j0 + TY >= P.ny;
-  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true>(P, A, M, sm, cta);
-  else rhs_body<MODE, false>(P, A, M, sm, cta);
+  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true, WENO>(P, A, M, sm, cta);
+  else rhs_body<MODE, false, WENO>(P, A, M, sm, cta);
 }
 
 }  // namespace streams

@@ -510,9 +510,14 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   e = cudaMallocHost((void**)&c->h_sc, sizeof(DevScal));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_part, ((size_t)NDIAG * RGRID + 8) * sizeof(double));
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaMallocHost(diagnostics)"); }
-  e = cudaFuncSetAttribute(k_rhs<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
+  {
+    const int smem_rhs = SM_RHS_DOUBLES * (int)sizeof(double);
+    e = cudaFuncSetAttribute(k_rhs<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
+  }
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaFuncSetAttribute(k_rhs)"); }
   *out = c;
   return STREAMS_OK;
@@ -600,14 +605,8 @@ static int ensure_inflow(streams_ctx* c) {
   return STREAMS_OK;
 }
 
-// node flags k_rhs has just written -> one bit per node (a3).  On a z-slab the caller now swaps the flag words of the
-// three planes next to each BC_HALO face (streams_flag_halo_*) before run_list.
-static int run_flag_pack(streams_ctx* c) {
-  k_flag_pack<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, c->nflag, c->fbits);
-  LAUNCH_CHECK("k_flag_pack");
-  return STREAMS_OK;
-}
-// lists of flagged interfaces and of the nodes next to them from the packed flags
+// lists of flagged interfaces and of the nodes next to them from the flag words k_rhs has just written (a3); on a z-slab
+// the caller has swapped the words of the three planes next to each BC_HALO face in between (streams_flag_halo_*)
 static int run_list(streams_ctx* c) {
   CK(cudaMemsetAsync(&c->sc->max_theta, 0, sizeof(double) + 3 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->st));
   CK(cudaMemsetAsync(&c->sc->icount[0], 0, 4 * sizeof(unsigned int), c->st));
@@ -637,16 +636,19 @@ static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, d
 static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in, dim3 grid) {
   RhsArgs A = A_in;
   A.use_tma = c->use_tma;
-  A.nflag = c->p.weno_enable ? c->nflag : nullptr;
+  A.fbits = c->p.weno_enable ? c->fbits : nullptr;
   const int qi = A.q == c->qbuf[1] ? 1 : 0;
   RhsMaps tm;
   tm.tile = c->tmap[qi]; tm.own = c->tmap_own[qi];
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
-  if (mode == 2) k_rhs<2><<<grid, NT, smem, c->st>>>(c->P, A, tm);       // fused RK stage, lazy forcing
-  else if (mode == 1) k_rhs<1><<<grid, NT, smem, c->st>>>(c->P, A, tm);  // fused RK stage
-  else k_rhs<0><<<grid, NT, smem, c->st>>>(c->P, A, tm);                 // residual only
+  const bool wn = A.fbits != nullptr;                                     // hybrid switch on: the kernel writes the flag words
+  if (mode == 2) k_rhs<2, false><<<grid, NT, smem, c->st>>>(c->P, A, tm);                // fused RK stage, lazy forcing (never with WENO)
+  else if (mode == 1 && wn) k_rhs<1, true><<<grid, NT, smem, c->st>>>(c->P, A, tm);      // fused RK stage
+  else if (mode == 1) k_rhs<1, false><<<grid, NT, smem, c->st>>>(c->P, A, tm);
+  else if (wn) k_rhs<0, true><<<grid, NT, smem, c->st>>>(c->P, A, tm);                   // residual only
+  else k_rhs<0, false><<<grid, NT, smem, c->st>>>(c->P, A, tm);
   LAUNCH_CHECK("k_rhs");
   if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
@@ -679,7 +681,6 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   A.partial = partial_ok ? c->partial : nullptr;
   if ((rc = launch_rhs(c, 0, A, c->rhs_grid))) return rc;
   if (c->p.weno_enable) {
-    if ((rc = run_flag_pack(c))) return rc;
     if ((rc = run_weno(c, w, d_rhs, nullptr, 0.0))) return rc;
   }
   if (c->p.forcing) {
@@ -758,13 +759,11 @@ static int do_stage_rhs(streams_ctx* c, int l, int part, bool single) {
     const bool partial_ok = !c->p.weno_enable;
     A.out_rhs = c->S[c->scur ^ 1]; A.partial = partial_ok ? c->partial : nullptr;
     if (any && (rc = launch_rhs(c, 0, A, grid))) return rc;
-    if (last && c->p.weno_enable && (rc = run_flag_pack(c))) return rc;
   } else {
     // fused: w_new = w + dt (alpha S + beta R) written to the other state buffer, S updated in place
     // R of the last stage is never read (alpha_0 = 0): neither this kernel nor k_weno_apply stores it
     A.q_out = c->qbuf[c->cur ^ 1]; A.S_prev = c->S[0]; A.S_out = c->S[0]; A.write_S = l < 2 ? 1 : 0;
     if (any && (rc = launch_rhs(c, 1, A, grid))) return rc;
-    if (last && c->p.weno_enable && (rc = run_flag_pack(c))) return rc;
   }
   return STREAMS_OK;
 }
