@@ -373,10 +373,12 @@ __device__ __noinline__ F5 wall_y(const DevP& P, const double* __restrict__ t, i
 // viscous terms on: every such test folds at compile time and no out-of-line call remains in the plane loop, which
 // frees ~30 registers for the scheduler.  Ghost slots (periodic wrap, reflection, ...) are handled in both.
 // MODE: 0 = residual only (streams_rhs), 1 = fused RK stage, 2 = fused RK stage with lazy forcing (mu(T) left to k_force_fix)
-template <int MODE, bool PLAIN, bool WENO>
+template <int MODE, bool PLAIN, bool WENO, int STAGE>
 __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const RhsMaps& M, double* sm, const int3 cta) {
   const CUtensorMap& tmap = M.tile;
   constexpr bool FUSED = MODE != 0, LAZY = MODE == 2;
+  // STAGE (fused launches): 0 = first RK stage (alpha = 0: no R_prev), 1 = middle, 2 = last (R is not stored: never read)
+  constexpr bool HAS_PREV = FUSED && STAGE > 0, WRITE_S = STAGE < 2, HAS_FPREV = LAZY && STAGE > 0;
   double* tiles = sm;
   double* stg = tiles + SM_TILES;
   double* gring = stg + 2 * SM_STG1;
@@ -506,7 +508,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
   double* scal = red + SM_RED + NBUF + 2;
   if (FUSED && tid == 0) {
     scal[0] = *A.dt_ptr;
-    scal[1] = A.f_prev && A.alpha != 0.0 ? *A.f_prev : 0.0;
+    scal[1] = HAS_FPREV ? *A.f_prev : 0.0;
   }
   __syncthreads();
   int slot7 = 0, b3 = 0;                                 // it % 7, it % 3
@@ -527,7 +529,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 #pragma unroll
       for (int f = 0; f < NF; ++f) cp_async8(d + f * NPT * 8, q + f * P.QS);
     }
-    if (FUSED && A.alpha != 0.0 && active && s - 2 >= k0 && s - 2 < k1) {
+    if (HAS_PREV && active && s - 2 >= k0 && s - 2 < k1) {
       // R_prev (and u_prev for the lazy forcing) of plane s-2, read in the NEXT step's epilogue (one step of slack:
       // the epilogue sits before the plane barrier and must not wait for HBM).  Thread-private slots: a thread's own
       // program order keeps the copy behind its reads of the slot, which happen between barrier arrive and wait.
@@ -536,7 +538,7 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
       const unsigned d = smem_u32(spring + tid) + (((it + 1) & 1) * 6 * NPT) * 8;
 #pragma unroll
       for (int v = 0; v < 5; ++v) cp_async8(d + v * NPT * 8, sp + v * P.N);
-      if (A.f_prev) cp_async8(d + 5 * NPT * 8, (A.q_out + zo + P.QS) + own32);
+      if (HAS_FPREV) cp_async8(d + 5 * NPT * 8, (A.q_out + zo + P.QS) + own32);
     }
     cp_async_commit();
     cp_async_wait<1>();                                  // the groups of steps <= s-1 have landed: R_prev of plane s-3 (and
@@ -743,12 +745,12 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
         const double* pv = spring + (it & 1) * 6 * NPT + tl;        // requested at the top of step s-1
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
-          double sp = A.alpha != 0.0 ? pv[v * NPT] : 0.0;
+          double sp = HAS_PREV ? pv[v * NPT] : 0.0;
           if (v == 1) sp += fprev;
-          if (v == 4 && A.f_prev && A.alpha != 0.0) sp = fma(fprev, pv[5 * NPT], sp);
-          dW[v] = dt * (A.alpha * sp + A.beta * R[v]);
+          if (v == 4 && HAS_FPREV) sp = fma(fprev, pv[5 * NPT], sp);
+          dW[v] = HAS_PREV ? dt * (A.alpha * sp + A.beta * R[v]) : dt * (A.beta * R[v]);
         }
-        if (A.write_S) {
+        if (WRITE_S) {
           double* so = (A.S_out + zo) + own32;
 #pragma unroll
           for (int v = 0; v < 5; ++v) so[v * P.N] = R[v];
@@ -821,7 +823,9 @@ __device__ __forceinline__ void rhs_body(const DevP& P, const RhsArgs& A, const 
 
 // WENO: the hybrid switch is on (the kernel also writes the node flag words); a template parameter, so that the flag code
 // does not exist in the launches of the central-only configs (it cost them 1.7 % as a run-time branch)
-template <int MODE, bool WENO>
+// STAGE: the RK stage of a fused launch (0, 1, 2; residual-only launches use 0): whether R_prev exists and whether R is
+// stored are compile-time facts of the launch
+template <int MODE, bool WENO, int STAGE>
 __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, const RhsArgs A, const __grid_constant__ RhsMaps M) {
   extern __shared__ __align__(128) double sm[];
   // CTA -> (tile, chunk): the chunk index varies fastest with the launch order, so that the CTAs resident at any time
@@ -834,8 +838,8 @@ __global__ void __launch_bounds__(NT, 1) k_rhs(const __grid_constant__ DevP P, c
   const bool outflow = P.bc[1] == BC_OUTFLOW && i0 + TX >= P.nx;
   const bool wall_lo = (P.bc[2] == BC_WALL_STAG || node_wall(P.bc[2])) && j0 == 0;
   const bool wall_hi = (P.bc[3] == BC_WALL_STAG || node_wall(P.bc[3]) || P.bc[3] == BC_OUTFLOW) && j0 + TY >= P.ny;
-  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true, WENO>(P, A, M, sm, cta);
-  else rhs_body<MODE, false, WENO>(P, A, M, sm, cta);
+  if (inside && A.use_tma && P.viscous && !outflow && !wall_lo && !wall_hi) rhs_body<MODE, true, WENO, STAGE>(P, A, M, sm, cta);
+  else rhs_body<MODE, false, WENO, STAGE>(P, A, M, sm, cta);
 }
 
 }  // namespace streams

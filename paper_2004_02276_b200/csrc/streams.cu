@@ -273,6 +273,19 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   return L;
 }
 
+// the instantiations of the fused kernel: mode (0 residual only, 1 fused RK stage, 2 fused stage with lazy forcing),
+// hybrid switch, RK stage.  Lazy forcing never runs with the hybrid switch; residual-only launches have no stage.
+typedef void (*RhsKernel)(const DevP, const RhsArgs, const RhsMaps);
+RhsKernel rhs_kernel(int mode, bool weno, int stage) {
+  if (mode == 0) return stage != 0 ? nullptr : (weno ? (RhsKernel)k_rhs<0, true, 0> : (RhsKernel)k_rhs<0, false, 0>);
+  if (mode == 2) {
+    if (weno) return nullptr;
+    return stage == 0 ? (RhsKernel)k_rhs<2, false, 0> : (stage == 1 ? (RhsKernel)k_rhs<2, false, 1> : (RhsKernel)k_rhs<2, false, 2>);
+  }
+  if (weno) return stage == 0 ? (RhsKernel)k_rhs<1, true, 0> : (stage == 1 ? (RhsKernel)k_rhs<1, true, 1> : (RhsKernel)k_rhs<1, true, 2>);
+  return stage == 0 ? (RhsKernel)k_rhs<1, false, 0> : (stage == 1 ? (RhsKernel)k_rhs<1, false, 1> : (RhsKernel)k_rhs<1, false, 2>);
+}
+
 int rgrid_for(long long N) { return (int)std::min<long long>(RGRID, (N + RT - 1) / RT); }
 
 }  // namespace
@@ -510,14 +523,12 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   e = cudaMallocHost((void**)&c->h_sc, sizeof(DevScal));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_part, ((size_t)NDIAG * RGRID + 8) * sizeof(double));
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaMallocHost(diagnostics)"); }
-  {
-    const int smem_rhs = SM_RHS_DOUBLES * (int)sizeof(double);
-    e = cudaFuncSetAttribute(k_rhs<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_rhs);
-  }
+  e = cudaSuccess;
+  for (int m = 0; m < 3 && e == cudaSuccess; ++m)
+    for (int w = 0; w < 2 && e == cudaSuccess; ++w)
+      for (int st = 0; st < 3 && e == cudaSuccess; ++st)
+        if (RhsKernel k = rhs_kernel(m, w != 0, st))
+          e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_RHS_DOUBLES * (int)sizeof(double));
   if (e != cudaSuccess) { cudaFree(c->small_dev); delete c; return cuda_fail(nullptr, e, "cudaFuncSetAttribute(k_rhs)"); }
   *out = c;
   return STREAMS_OK;
@@ -643,12 +654,9 @@ static int launch_rhs(streams_ctx* c, int mode, const RhsArgs& A_in, dim3 grid) 
   const size_t smem = SM_RHS_DOUBLES * sizeof(double);
   const bool rec = c->prof_on && c->prof_n < 4096;
   if (rec) CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->st));
-  const bool wn = A.fbits != nullptr;                                     // hybrid switch on: the kernel writes the flag words
-  if (mode == 2) k_rhs<2, false><<<grid, NT, smem, c->st>>>(c->P, A, tm);                // fused RK stage, lazy forcing (never with WENO)
-  else if (mode == 1 && wn) k_rhs<1, true><<<grid, NT, smem, c->st>>>(c->P, A, tm);      // fused RK stage
-  else if (mode == 1) k_rhs<1, false><<<grid, NT, smem, c->st>>>(c->P, A, tm);
-  else if (wn) k_rhs<0, true><<<grid, NT, smem, c->st>>>(c->P, A, tm);                   // residual only
-  else k_rhs<0, false><<<grid, NT, smem, c->st>>>(c->P, A, tm);
+  // instantiation: mode, hybrid switch (the kernel writes the flag words), RK stage (0: alpha = 0, no R_prev; 2: R not stored)
+  const int stage = mode == 0 ? 0 : (A.alpha == 0.0 ? 0 : (A.write_S ? 1 : 2));
+  rhs_kernel(mode, A.fbits != nullptr, stage)<<<grid, NT, smem, c->st>>>(c->P, A, tm);
   LAUNCH_CHECK("k_rhs");
   if (rec) { CK(cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->st)); c->prof_n++; }
   return STREAMS_OK;
