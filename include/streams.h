@@ -254,6 +254,26 @@ int streams_profile_read(streams_ctx* ctx, double* h_ms_total, long long* h_laun
  * Not part of the method (PAPER.md gives no peak); used by bench.py next to MEASURED_PEAKS.json. */
 int streams_fp64_peak(void* cuda_stream, double* h_tinstr);
 
+/* The S10 maxima (PAPER.md:89-99 is silent on the time step; north_star "CFL reduction", S10)
+ * WITHOUT ANY ALLOCATION, for callers that cannot allocate (CUDA graph capture, serving loops): the maxima over the
+ * nodes of (|u_d| + c) / h_d, d = x, y, z, of the conservative state d_w (device, [5][nz][ny][nx], caller-owned, read
+ * only; any state of the context's grid, not necessarily the one set by streams_set_state) are written to d_speeds
+ * (device, 3 doubles, caller-owned) by ONE kernel enqueued on the context stream (asynchronous); the time step of
+ * S10 is cfl / max(d_speeds[0..2]).  Same numbers as streams_diagnostics().max_speed of that state.  The grid
+ * metrics and gas constants are the context's; the per-CTA partial maxima and the "last CTA" ticket live in a
+ * file-scope `static __device__` array of the library (98 560 bytes: 3 x 4096 doubles + a 256-byte ticket line; every
+ * GPU that loads the library holds it until exit), NOT in the workspace.  Calls neither cudaMalloc / cudaFree nor any
+ * allocating routine; the first call on a device resolves the array's device address (cudaGetSymbolAddress, no
+ * allocation: make it once before a capture starts), later calls enqueue one 4-byte memset (the ticket must start at
+ * zero) and the kernel.
+ * Limit: one CTA reduces 8192 nodes and the array holds 4096 CTAs: grids of more than STREAMS_STATIC_MAX_NODES nodes
+ * are rejected with STREAMS_EINVAL ("... exceeds the static scratch limit ...") before anything is enqueued.
+ * Every call on a device, of every context, shares the one array: calls that OVERLAP on the GPU (different
+ * streams, no ordering between them) race on it and return garbage; calls on one stream, or ordered by events, are safe.
+ * STREAMS_EINVAL for null arguments; STREAMS_ECUDA for a CUDA failure. */
+#define STREAMS_STATIC_MAX_NODES 33554432LL
+int streams_max_speed_static(streams_ctx* ctx, const double* d_w, double* d_speeds);
+
 /* Number of kernel launches enqueued by this context so far (for bench accounting). */
 long long streams_launch_count(const streams_ctx* ctx);
 

@@ -18,7 +18,8 @@ EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "st
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
            "streams_diagnostics", "streams_step_begin", "streams_stage_rhs", "streams_stage_end", "streams_reduce_ptr",
            "streams_halo_bytes", "streams_halo_pack", "streams_halo_unpack", "streams_flag_halo_bytes", "streams_flag_halo_pack",
-           "streams_flag_halo_unpack", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_launch_count", "streams_last_error", "streams_destroy"]
+           "streams_flag_halo_unpack", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_max_speed_static",
+           "streams_launch_count", "streams_last_error", "streams_destroy"]
 
 
 class StreamsGrid(C.Structure):
@@ -93,6 +94,7 @@ def lib():
         L.streams_profile.argtypes = [C.c_void_p, C.c_int]
         L.streams_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.streams_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.streams_max_speed_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.streams_launch_count.argtypes = [C.c_void_p]
         L.streams_launch_count.restype = C.c_longlong
         L.streams_last_error.argtypes = [C.c_void_p]
@@ -276,6 +278,7 @@ class Streams:
     # --- staged stepping and z-slab halos (include/streams.h) ------------
     PART_ALL, PART_INTERIOR, PART_BOUNDARY = 0, 1, 2
     FACE_ZMIN, FACE_ZMAX = 4, 5
+    STATIC_MAX_NODES = 33554432          # streams_max_speed_static (include/streams.h)
 
     def step_begin(self):
         self._chk(lib().streams_step_begin(self._h))
@@ -336,6 +339,15 @@ class Streams:
         rc = lib().streams_diagnostics(self._h, C.byref(d))
         self._chk(rc, allow=() if check else (STREAMS_ENONFINITE,))
         return d
+
+    def max_speed_static(self, w, out):
+        """S10 maxima of the conservative state `w` ([5][nz][ny][nx], device) into `out` (3 doubles, device), asynchronous
+        on the context stream; the library call allocates nothing (its scratch is a static device array; grids of at most
+        STATIC_MAX_NODES nodes).  Both tensors are the caller's: nothing is allocated here either."""
+        self._pre(w)
+        self._chk(lib().streams_max_speed_static(self._h, self._dev(w, self.shape), self._dev(out, (3,))))
+        self._post(out)
+        return out
 
     # --- statistics (PAPER.md:103) --------------------------------------------------------------
     def stats_accumulate(self):

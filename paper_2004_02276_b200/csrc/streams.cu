@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1049,3 +1050,98 @@ int streams_diagnostics(streams_ctx* c, streams_diag* out) {
 }
 
 }  // extern "C"
+
+// ---- S10 maxima without any allocation (include/streams.h, streams_max_speed_static) --------------------------------
+// The scratch of this ONE entry point is a file-scope device array instead of caller workspace: per-CTA partial maxima
+// [3][STATIC_MAX_CTAS] followed by a 256-byte line whose first word is the "CTAs finished" ticket.  Every device that
+// loads the library holds the 98 560 bytes until exit; all calls on a device share it (overlapping calls race) and it
+// keeps the last call's contents: the partials are overwritten before they are read, the ticket is zeroed before each
+// launch.  In HOST code the array's name is a host-side stand-in, not a device address: static_scratch() resolves the
+// address once per device with cudaGetSymbolAddress and the kernel takes it as an argument.
+namespace {
+constexpr int STATIC_CHUNK = RT * 32;           // nodes reduced by one CTA
+constexpr int STATIC_MAX_CTAS = 4096;
+constexpr int STATIC_WORDS = 3 * STATIC_MAX_CTAS + 32;
+static_assert((long long)STATIC_CHUNK * STATIC_MAX_CTAS == STREAMS_STATIC_MAX_NODES, "streams.h states the limit");
+constexpr int STATIC_MAX_DEV = 64;
+}  // namespace
+
+static __device__ __align__(256) double g_static_scratch[STATIC_WORDS];
+
+namespace {
+// one CTA = STATIC_CHUNK consecutive nodes of the conservative state; the last CTA to finish (ticket) reduces the
+// partials and writes the three maxima.  The maximum is exact, so the result does not depend on the CTA order.
+__global__ void __launch_bounds__(RT) k_speed_static(const __grid_constant__ DevP P, const double* __restrict__ w,
+                                                     double* scratch, double* __restrict__ out) {
+  __shared__ double sh[RT / 32];
+  __shared__ int is_last;
+  double m[3] = {0.0, 0.0, 0.0};
+  const long long o0 = blockIdx.x * (long long)STATIC_CHUNK;
+  const long long o1 = o0 + STATIC_CHUNK < P.N ? o0 + STATIC_CHUNK : P.N;
+  for (long long o = o0 + threadIdx.x; o < o1; o += RT) {
+    int i, j, k;
+    node_ijk(P, o, i, j, k);
+    Prim q;
+    cons2prim(P, w[o], w[o + P.N], w[o + 2 * P.N], w[o + 3 * P.N], w[o + 4 * P.N], q);      // S3 (mu is not used)
+    const double cs = sqrt(P.gam * P.Rgas * q.T);
+    m[0] = fmax(m[0], (fabs(q.u) + cs) * P.ih[0][i]);
+    m[1] = fmax(m[1], (fabs(q.v) + cs) * P.ih[1][j]);
+    m[2] = fmax(m[2], (fabs(q.w) + cs) * P.ih[2][k]);
+  }
+  for (int d = 0; d < 3; ++d) {
+    const double t = block_max<RT>(m[d], sh, threadIdx.x);
+    if (threadIdx.x == 0) scratch[d * STATIC_MAX_CTAS + blockIdx.x] = t;
+  }
+  unsigned int* ticket = reinterpret_cast<unsigned int*>(scratch + 3 * STATIC_MAX_CTAS);
+  if (threadIdx.x == 0) {
+    __threadfence();                                              // the partials are visible before the ticket moves
+    is_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  const volatile double* part = scratch;
+  for (int d = 0; d < 3; ++d) {
+    double mm = 0.0;
+    for (int e = threadIdx.x; e < (int)gridDim.x; e += RT) mm = fmax(mm, part[d * STATIC_MAX_CTAS + e]);
+    const double t = block_max<RT>(mm, sh, threadIdx.x);
+    if (threadIdx.x == 0) out[d] = t;
+  }
+  if (threadIdx.x == 0) *ticket = 0u;                             // left at zero for the next call
+}
+
+// device address of g_static_scratch on `device` (current), resolved once per device
+int static_scratch(streams_ctx* c, int device, double** ptr) {
+  static double* addr[STATIC_MAX_DEV];
+  static std::mutex mu;
+  if (device < 0 || device >= STATIC_MAX_DEV) return fail(c, STREAMS_EINVAL, "streams_max_speed_static: device index beyond 63");
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[device]) {
+    double* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_static_scratch);
+    if (e != cudaSuccess || !p) return cuda_fail(c, e, "cudaGetSymbolAddress(g_static_scratch)");
+    addr[device] = p;
+  }
+  *ptr = addr[device];
+  return STREAMS_OK;
+}
+}  // namespace
+
+extern "C" int streams_max_speed_static(streams_ctx* c, const double* d_w, double* d_speeds) {
+  if (!c || !d_w || !d_speeds) return fail(c, STREAMS_EINVAL, "null argument");
+  if (c->P.N > STREAMS_STATIC_MAX_NODES) {
+    char b[200];
+    snprintf(b, sizeof b, "streams_max_speed_static: %lld nodes exceeds the static scratch limit of %lld nodes (use streams_diagnostics)",
+             (long long)c->P.N, (long long)STREAMS_STATIC_MAX_NODES);
+    return fail(c, STREAMS_EINVAL, b);
+  }
+  DevGuard dg(c->device);
+  double* scratch = nullptr;
+  int rc;
+  if ((rc = static_scratch(c, c->device, &scratch))) return rc;
+  const int grid = (int)((c->P.N + STATIC_CHUNK - 1) / STATIC_CHUNK);
+  CK(cudaMemsetAsync(scratch + 3 * STATIC_MAX_CTAS, 0, sizeof(unsigned int), c->st));
+  k_speed_static<<<grid, RT, 0, c->st>>>(c->P, d_w, scratch, d_speeds);
+  LAUNCH_CHECK("k_speed_static");
+  return STREAMS_OK;
+}
