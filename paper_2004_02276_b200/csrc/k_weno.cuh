@@ -99,19 +99,33 @@ __device__ __forceinline__ int row_of(const DevP& P, int j, int k) {
   return kk * P.ny + jj;
 }
 
+// Warp-cooperative append: every lane holds the bit word of ITS 32 nodes (`bits`), the list position of its first entry
+// (`pos`) and its first node (`o0`); the warp walks the non-empty words and lane b writes the entry of node b, so that one
+// store instruction writes consecutive entries (a thread writing its own run costs one sector per entry).
+template <class F>
+__device__ __forceinline__ void warp_emit(unsigned int bits, unsigned int pos, unsigned int o0, int lane, F&& store) {
+  for (unsigned int todo = __ballot_sync(0xffffffffu, bits != 0u); todo; todo &= todo - 1) {
+    const int src = __ffs(todo) - 1;
+    const unsigned int b = __shfl_sync(0xffffffffu, bits, src), p0 = __shfl_sync(0xffffffffu, pos, src);
+    const unsigned int on = __shfl_sync(0xffffffffu, o0, src);
+    if ((b >> lane) & 1u) store(on + (unsigned int)lane, p0 + (unsigned int)__popc(b & ((1u << lane) - 1u)));
+  }
+}
+
 // Interface flags and lists from the packed node flags, ONE THREAD PER WORD (32 nodes of a row): interface i+1/2 along
 // d is flagged iff any of nodes i-2..i+3 is (A6), i.e. an OR of six shifted words (x) or of six words of neighbouring
 // rows / planes (y, z).  Entries: node list (node index + 6-bit mask, bit 2d = interface below, 2d+1 = above) of the
 // nodes with a flagged interface, and per direction the list of flagged interfaces by their lower node (the interface
-// below the first node of a non-periodic direction: node | IFACE_BELOW).  A warp reserves its slots with one atomic
-// per list; inside a warp the entries follow the words, i.e. x, so that the consumers read their stencils coalesced.
+// below the first node of a non-periodic direction: node | IFACE_BELOW).  A CTA reserves its slots with one atomic
+// per list and round; inside a CTA the entries follow the words, i.e. x, so that the consumers read their stencils coalesced.
 __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P, const unsigned int* __restrict__ fbits,
                                                   unsigned int* __restrict__ list, unsigned char* __restrict__ lmask,
                                                   unsigned int* __restrict__ ilist /* [3][istride] or NULL */, size_t istride,
                                                   unsigned char* __restrict__ iflags_out /* [3][N] or NULL */, DevScal* sc) {
   const int nw = words_per_row(P);
   const unsigned int nwords = (unsigned int)(P.ny * P.nz) * (unsigned int)nw;
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __shared__ unsigned int s_wtot[2][4][RT / 32], s_base[2][4];
   unsigned long long cnt[3] = {0, 0, 0};
   const unsigned int nround = (nwords + gridDim.x * RT - 1) / (gridDim.x * RT);
   for (unsigned int it = 0; it < nround; ++it) {
@@ -178,53 +192,72 @@ __global__ void __launch_bounds__(RT) k_weno_list(const __grid_constant__ DevP P
       }
     }
     const unsigned int o0 = row * (unsigned int)P.nx + i0;           // node of bit 0 (N < 2^31 with the switch on)
-    // ---- interface lists
+    // ---- entries of this word in the four lists (0..2: interfaces along d, 3: nodes)
+    unsigned int lb[3] = {0, 0, 0};                                  // below-entries: first node of a non-periodic direction
+    if (in && ilist) {
+      if (P.bc[0] != BC_PERIODIC && i0 == 0) lb[0] = lo[0] & 1u;
+      if (P.bc[2] != BC_PERIODIC && j == 0) lb[1] = lo[1];
+      if (P.bc[4] != BC_PERIODIC && k == 0) lb[2] = lo[2];
+    }
+    const unsigned int any = (in && list) ? (lo[0] | hi[0] | lo[1] | hi[1] | lo[2] | hi[2]) : 0u;
+    unsigned int n_me[4], pre[4];
+#pragma unroll
+    for (int l = 0; l < 3; ++l) n_me[l] = (in && ilist) ? (unsigned int)(__popc(hi[l]) + __popc(lb[l])) : 0u;
+    n_me[3] = (unsigned int)__popc(any);
+    // The CTA reserves its slots with ONE atomic per list and round (a warp-wise reservation made 4 x 32 768 atomics on
+    // four neighbouring counters for config 4: the kernel ran at the rate of same-address atomics).  Two sets of the
+    // shared counters alternate between rounds, so that a warp that runs ahead cannot overwrite what a slower one reads.
+    unsigned int* wt = s_wtot[it & 1][0];
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      unsigned int v = n_me[l];                                      // inclusive warp prefix sum
+#pragma unroll
+      for (int sft = 1; sft < 32; sft <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, v, sft); if (lane >= sft) v += t; }
+      pre[l] = v;
+      if (lane == 31) wt[l * (RT / 32) + wid] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+      unsigned int tot = 0;
+#pragma unroll
+      for (int w = 0; w < RT / 32; ++w) tot += wt[threadIdx.x * (RT / 32) + w];
+      unsigned int* counter = threadIdx.x < 3 ? &sc->icount[threadIdx.x] : &sc->list_count;
+      s_base[it & 1][threadIdx.x] = tot ? atomicAdd(counter, tot) : 0u;
+    }
+    __syncthreads();
+    unsigned int pos[4];
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      unsigned int base = s_base[it & 1][l];
+      for (int w = 0; w < wid; ++w) base += wt[l * (RT / 32) + w];
+      pos[l] = base + pre[l] - n_me[l];
+    }
+    // ---- interface lists: the warp writes the entries of one word at a time (lane b = node b of the word)
     if (ilist) {
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        // below-entries: first node of a non-periodic direction
-        unsigned int lb = 0;
-        if (in && P.bc[2 * d] != BC_PERIODIC) {
-          if (d == 0) lb = i0 == 0 ? (lo[0] & 1u) : 0u;
-          else if (d == 1) lb = j == 0 ? lo[1] : 0u;
-          else lb = k == 0 ? lo[2] : 0u;
-        }
-        const unsigned int n_me = in ? (unsigned int)(__popc(hi[d]) + __popc(lb)) : 0u;
-        unsigned int pre = n_me;                                     // inclusive warp prefix sum
-#pragma unroll
-        for (int sft = 1; sft < 32; sft <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, pre, sft); if (lane >= sft) pre += t; }
-        const unsigned int tot = __shfl_sync(0xffffffffu, pre, 31);
-        unsigned int base = 0;
-        if (tot) {
-          if (lane == 31) base = atomicAdd(&sc->icount[d], tot);
-          base = __shfl_sync(0xffffffffu, base, 31);
-        }
-        unsigned int pos = base + pre - n_me;
         unsigned int* li = ilist + d * istride;
-        for (unsigned int m = hi[d]; m; m &= m - 1) li[pos++] = o0 + (unsigned int)(__ffs(m) - 1);
-        for (unsigned int m = lb; m; m &= m - 1) li[pos++] = (o0 + (unsigned int)(__ffs(m) - 1)) | IFACE_BELOW;
+        warp_emit(hi[d], pos[d], o0, lane, [&](unsigned int node, unsigned int at) { li[at] = node; });
+        warp_emit(lb[d], pos[d] + (unsigned int)__popc(hi[d]), o0, lane, [&](unsigned int node, unsigned int at) { li[at] = node | IFACE_BELOW; });
       }
     }
     // ---- node list
     if (list) {
-      const unsigned int any = in ? (lo[0] | hi[0] | lo[1] | hi[1] | lo[2] | hi[2]) : 0u;
-      const unsigned int n_me = (unsigned int)__popc(any);
-      unsigned int pre = n_me;
+      for (unsigned int todo = __ballot_sync(0xffffffffu, any != 0u); todo; todo &= todo - 1) {
+        const int src = __ffs(todo) - 1;
+        const unsigned int bw = __shfl_sync(0xffffffffu, any, src), p0 = __shfl_sync(0xffffffffu, pos[3], src);
+        const unsigned int on = __shfl_sync(0xffffffffu, o0, src);
+        unsigned int m = 0;
 #pragma unroll
-      for (int sft = 1; sft < 32; sft <<= 1) { const unsigned int t = __shfl_up_sync(0xffffffffu, pre, sft); if (lane >= sft) pre += t; }
-      const unsigned int tot = __shfl_sync(0xffffffffu, pre, 31);
-      unsigned int base = 0;
-      if (tot) {
-        if (lane == 31) base = atomicAdd(&sc->list_count, tot);
-        base = __shfl_sync(0xffffffffu, base, 31);
-      }
-      unsigned int pos = base + pre - n_me;
-      for (unsigned int m = any; m; m &= m - 1) {
-        const int b = __ffs(m) - 1;
-        list[pos] = o0 + (unsigned int)b;
-        lmask[pos] = (unsigned char)(((lo[0] >> b) & 1u) | (((hi[0] >> b) & 1u) << 1) | (((lo[1] >> b) & 1u) << 2) |
-                                     (((hi[1] >> b) & 1u) << 3) | (((lo[2] >> b) & 1u) << 4) | (((hi[2] >> b) & 1u) << 5));
-        ++pos;
+        for (int d = 0; d < 3; ++d) {
+          m |= ((__shfl_sync(0xffffffffu, lo[d], src) >> lane) & 1u) << (2 * d);
+          m |= ((__shfl_sync(0xffffffffu, hi[d], src) >> lane) & 1u) << (2 * d + 1);
+        }
+        if ((bw >> lane) & 1u) {
+          const unsigned int at = p0 + (unsigned int)__popc(bw & ((1u << lane) - 1u));
+          list[at] = on + (unsigned int)lane;
+          lmask[at] = (unsigned char)m;
+        }
       }
     }
   }
