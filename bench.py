@@ -371,7 +371,7 @@ def run_ours(args, rank, world, local_rank):
                             "launches_timed": int(rhs_n), "avg_launch_ms": rhs_avg_ms,
                             "share_of_step": rhs_share, "launch_times_from": "timed region" if prof_in_region else "separate profiled pass (timed region replays CUDA graphs)",
                             "bound_times_ms": {"alu": 1e3 * t_alu, "hbm": 1e3 * t_hbm},
-                            "limiter_observed": "neither roofline binds: fp64 pipe 47 %, issue slots 51 %, shared-memory pipe 60 % at "
+                            "limiter_observed": "neither roofline binds: fp64 pipe 51 %, issue slots 52 %, shared-memory pipe 63 % at "
                                                 "8 warps/SM; largest stall = fixed-latency dependencies (profiles/r02_*_k_rhs_config5.md)",
                             "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                                     "peak_source": peak_src, "bytes_per_point_by_stage": stage_bytes,

@@ -239,13 +239,18 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   }
   const int tiles_x = (g.nx + TX - 1) / TX, tiles_y = (g.ny + TY - 1) / TY;
   const int tiles = tiles_x * tiles_y;
-  // planes per CTA.  Grids with at least half a wave of tiles (148 SMs, one CTA each): about two waves of CTAs, chunks
-  // of at most LZ_MAX planes, the 6 ghost planes of a chunk amortised over >= 8 planes (measured on configs 3-5: CTAs
-  // at different z also spread the DRAM traffic better than one wave marching in lockstep).  Smaller grids cannot fill
-  // the SMs with tiles: there the chunk count minimises  waves x (lz + 3.5)  (ghost planes cost ~40 % of a full one).
+  // planes per CTA.  Grids with at least half a wave of tiles (148 SMs, one CTA each): a launch takes about
+  //   (tiles c / 148) (nz / c + G) + kappa (nz / c + G),   c chunks of nz / c planes, G ~ the cost of a chunk's 6 ghost planes,
+  // the second term being the tail: CTAs differ (a wall tile takes twice the time of an interior one) and the last ones
+  // run on a partly empty GPU.  Minimum at c = sqrt(kappa 148 nz / (G tiles)); kappa / G = 0.43 fits the measured optima
+  // (sweep of c on one box: config 3 / 6 (128 tiles, nz 128) c = 8: -6 % per step against c = 3; config 4 (1024 tiles,
+  // nz 128) c = 2 ... 3: -3 % against c = 1; config 5 (2048 tiles, nz 512) c = 4 as before), chunks of at most LZ_MAX and
+  // at least 8 planes.  CTAs at different z also spread the DRAM traffic better than one wave marching in lockstep.
+  // Smaller grids cannot fill the SMs with tiles: there the chunk count minimises  waves x (lz + 3.5)  (ghost planes
+  // cost ~40 % of a full one; config 2: one wave of 128 CTAs beats every finer cut).
   int nchunk;
   if (tiles >= 74) {
-    nchunk = (2 * 148 + tiles - 1) / tiles;
+    nchunk = (int)std::lround(std::sqrt(0.43 * 148.0 * g.nz / tiles));
     nchunk = std::max(nchunk, (g.nz + LZ_MAX - 1) / LZ_MAX);
     nchunk = std::min(nchunk, std::max(1, g.nz / 8));
   } else {
