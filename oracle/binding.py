@@ -23,7 +23,7 @@ class OracleParams(C.Structure):
                 ("shock_angle_deg", C.c_double), ("x_shock", C.c_double), ("cfl", C.c_double),
                 ("dt_fixed", C.c_double),
                 ("visc_model", C.c_int), ("order", C.c_int), ("weno_enable", C.c_int), ("forcing", C.c_int),
-                ("viscous_enable", C.c_int), ("bc", C.c_int * 6), ("pad_", C.c_int)]
+                ("viscous_enable", C.c_int), ("bc", C.c_int * 6), ("weno_order", C.c_int)]
 
 
 class OracleDiag(C.Structure):
@@ -56,6 +56,8 @@ def lib():
         L.oracle_coeffs.argtypes = [C.c_int, _DBL, _DBL]
         L.oracle_weno5.argtypes = [C.c_double] * 5
         L.oracle_weno5.restype = C.c_double
+        L.oracle_weno3.argtypes = [C.c_double] * 3
+        L.oracle_weno3.restype = C.c_double
         L.oracle_eigen.argtypes = [C.c_int, C.c_double, _DBL, C.c_double, _DBL, _DBL, _DBL]
         L.oracle_eigen.restype = None
         L.oracle_shock_state.argtypes = [C.POINTER(OracleParams), _DBL, _DBL]
@@ -82,7 +84,7 @@ def make_params(params: dict) -> OracleParams:
     for name, _t in OracleParams._fields_:
         if name == "pad_":
             continue
-        v = params[name]
+        v = params.get("weno_order", 5) if name == "weno_order" else params[name]
         if isinstance(v, (list, tuple, np.ndarray)):
             arr = getattr(p, name)
             for i, x in enumerate(v):
@@ -101,6 +103,10 @@ def coeffs(order):
 
 def weno5(a, b, c, d, e):
     return lib().oracle_weno5(a, b, c, d, e)
+
+
+def weno3(a, b, c):
+    return lib().oracle_weno3(a, b, c)
 
 
 def eigen(d, gamma, ubar, Hbar):

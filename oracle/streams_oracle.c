@@ -181,6 +181,7 @@ static int check_params(const oracle_grid* g, const oracle_params* p) {
   if (!(p->gamma > 1.0) || !(p->Rgas > 0.0) || !(p->Pr > 0.0)) return 0;
   if (p->order != 2 && p->order != 4 && p->order != 6) return 0;
   if (p->weno_enable && !(p->sensor_eps > 0.0)) return 0;
+  if (p->weno_order != 0 && p->weno_order != 3 && p->weno_order != 5) return 0;
   const int n[3] = {g->nx, g->ny, g->nz};
   for (int d = 0; d < 3; ++d) {
     int lo = p->bc[2 * d], hi = p->bc[2 * d + 1];
@@ -481,6 +482,19 @@ double oracle_weno5(double a, double b, double cc, double d, double e) {
   return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
 }
 
+/* Variant (A23): WENO3 of Jiang & Shu (ref. [34]) -- two candidate stencils {a,b}, {b,c} for the
+ * interface right of b, linear weights 1/3, 2/3, smoothness (b-a)^2, (c-b)^2, same epsilon and exponent as the fifth-order one */
+double oracle_weno3(double a, double b, double cc) {
+  const double q0 = (-a + 3.0 * b) / 2.0;
+  const double q1 = (b + cc) / 2.0;
+  const double b0 = (b - a) * (b - a);
+  const double b1 = (cc - b) * (cc - b);
+  const double eps = 1e-6;
+  const double a0 = (1.0 / 3.0) / ((eps + b0) * (eps + b0));
+  const double a1 = (2.0 / 3.0) / ((eps + b1) * (eps + b1));
+  return (a0 * q0 + a1 * q1) / (a0 + a1);
+}
+
 /* S6 step 2: left/right eigenvectors of dF_d/dw in conservative variables, row-major 5x5 */
 void oracle_eigen(int d, double gam, const double ub[3], double Hb, double Lm[25], double Rm[25], double lam[5]) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
@@ -526,6 +540,7 @@ static void weno_flux(const oracle_ctx* c, int d, size_t o, double F[5]) {
   const size_t NP = c->NP, s = c->sd[d];
   const double gam = c->p.gamma;
   const double* Q = c->q;
+  const int w3 = c->p.weno_order == 3;
   /* 1. Roe state from nodes i, i+1 */
   const size_t oa = o, ob = o + s;
   const double ua[3] = {Q[Q_U * NP + oa], Q[Q_V * NP + oa], Q[Q_W * NP + oa]};
@@ -554,6 +569,8 @@ static void weno_flux(const oracle_ctx* c, int d, size_t o, double F[5]) {
       wc[qn][sc] = a1; fc[qn][sc] = a2;
     }
     const double lq[5] = {un - cs, un, un, un, un + cs};
+    /* local Lax-Friedrichs: maximum over the nodes the reconstruction reads (i-2..i+3 for WENO5, i-1..i+2 for WENO3, A23) */
+    if (w3 && (qn == 0 || qn == 5)) continue;
     for (int sc = 0; sc < 5; ++sc) if (fabs(lq[sc]) > al[sc]) al[sc] = fabs(lq[sc]);
   }
   /* 5.-6. split, reconstruct; 7. project back */
@@ -564,7 +581,8 @@ static void weno_flux(const oracle_ctx* c, int d, size_t o, double F[5]) {
       fp[qn] = 0.5 * (fc[qn][sc] + al[sc] * wc[qn][sc]);
       fm[qn] = 0.5 * (fc[qn][sc] - al[sc] * wc[qn][sc]);
     }
-    fh[sc] = oracle_weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + oracle_weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+    if (w3) fh[sc] = oracle_weno3(fp[1], fp[2], fp[3]) + oracle_weno3(fm[4], fm[3], fm[2]);
+    else fh[sc] = oracle_weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + oracle_weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
   }
   for (int v = 0; v < 5; ++v) {
     double acc = 0.0;

@@ -32,7 +32,7 @@ typedef struct {
   double shock_angle_deg, x_shock, cfl, dt_fixed;
   int visc_model, order, weno_enable, forcing, viscous_enable;
   int bc[6];
-  int pad_;
+  int weno_order; /* order of the WENO reconstruction on flagged interfaces: 5 (default; 0 means 5) or 3 (reading A23) */
 } oracle_params;
 
 typedef struct {
@@ -64,6 +64,7 @@ int  oracle_stats_reset(oracle_ctx*);
 /* pieces exposed so that tests can pin them one by one */
 int  oracle_coeffs(int order, double a_out[3], double b_out[3]);            /* a_l, b_l tables        */
 double oracle_weno5(double a, double b, double c, double d, double e);      /* S6 step 6               */
+double oracle_weno3(double a, double b, double c);                          /* A23: third-order variant */
 void oracle_eigen(int d, double gamma, const double ubar[3], double Hbar,
                   double Lm[25], double Rm[25], double lam[5]);             /* S6 step 2 (row-major)   */
 int  oracle_shock_state(const oracle_params*, double post_prim[5], double* beta_rad); /* S1 shock generator */

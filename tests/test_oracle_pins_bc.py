@@ -351,8 +351,9 @@ def test_roe_state_property_U(ob, d):
         assert np.abs(Rm2 @ np.diag(lam2) @ Lm2 @ (wb - wa) - rhs).max() > 1e-4 * np.abs(rhs).max()
 
 
+@pytest.mark.parametrize("order", [5, 3])
 @pytest.mark.parametrize("d", [0, 1, 2])
-def test_weno_flux_at_a_moving_shock_and_a_contact(ob, d):
+def test_weno_flux_at_a_moving_shock_and_a_contact(ob, d, order):
     """End to end through the oracle's WENO flux (every interface WENO).  Two uniform states that satisfy the
     Rankine-Hugoniot conditions of a shock of speed s: by property U the jump lies in ONE characteristic field of the
     Roe matrix, the other four fields are constant across the stencil, and the Lax-Friedrichs WENO flux at the jump is
@@ -364,7 +365,7 @@ def test_weno_flux_at_a_moving_shock_and_a_contact(ob, d):
     xs = np.arange(n) / n
     bc = [W.BC_PERIODIC] * 6
     bc[2 * d] = bc[2 * d + 1] = W.BC_EXTRAP
-    prm = W.default_params(Rgas=R_GAS, viscous_enable=0, weno_enable=1, sensor_threshold=-1.0, sensor_eps=1.0, bc=bc)
+    prm = W.default_params(Rgas=R_GAS, viscous_enable=0, weno_enable=1, sensor_threshold=-1.0, sensor_eps=1.0, bc=bc, weno_order=order)
     nn = [1, 1, 1]
     nn[d] = n
     coords = [np.zeros(1)] * 3

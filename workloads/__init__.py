@@ -23,7 +23,7 @@ def default_params(**over) -> dict:
              sensor_threshold=0.5, sensor_eps=1.0, T_wall=[1.0, 1.0], y_wall=[-1.0, 1.0],
              fs=[1.0, 0.0, 0.0, 0.0, 1.0], shock_angle_deg=0.0, x_shock=0.0, cfl=0.5, dt_fixed=0.0,
              visc_model=VISC_POWER, order=6, weno_enable=0, forcing=0, viscous_enable=1,
-             bc=[BC_PERIODIC] * 6)
+             bc=[BC_PERIODIC] * 6, weno_order=5)
     for k, v in over.items():
         if k not in p:
             raise KeyError(k)
