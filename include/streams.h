@@ -105,7 +105,9 @@ typedef struct {
   int forcing;             /* 1: constant bulk mass-flow forcing in x      */
   int viscous_enable;      /* 0: Euler equations (conservation / KE tests)                    */
   int bc[6];               /* STREAMS_BC_* for xmin,xmax,ymin,ymax,zmin,zmax                   */
-  int pad_;
+  int weno_order;          /* order of the WENO reconstruction on flagged interfaces (PAPER.md:77-79 names none): 5 =
+                            * Jiang-Shu WENO5 (default, the measured path; 0 means 5) or 3 (variant, A23: nodes
+                            * i-1..i+2, also for the Lax-Friedrichs maximum); the flag rule (six nodes) does not change */
 } streams_params;
 
 /* Reductions over the current state (and the last RHS evaluation). */

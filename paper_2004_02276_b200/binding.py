@@ -34,7 +34,7 @@ class StreamsParams(C.Structure):
                 ("shock_angle_deg", C.c_double), ("x_shock", C.c_double), ("cfl", C.c_double),
                 ("dt_fixed", C.c_double),
                 ("visc_model", C.c_int), ("order", C.c_int), ("weno_enable", C.c_int), ("forcing", C.c_int),
-                ("viscous_enable", C.c_int), ("bc", C.c_int * 6), ("pad_", C.c_int)]
+                ("viscous_enable", C.c_int), ("bc", C.c_int * 6), ("weno_order", C.c_int)]
 
 
 class StreamsDiag(C.Structure):
@@ -119,7 +119,7 @@ def make_params(params: dict) -> StreamsParams:
     for name, _t in StreamsParams._fields_:
         if name == "pad_":
             continue
-        v = params[name]
+        v = params.get("weno_order", 5) if name == "weno_order" else params[name]
         if isinstance(v, (list, tuple, np.ndarray)):
             arr = getattr(p, name)
             for i, x in enumerate(v):

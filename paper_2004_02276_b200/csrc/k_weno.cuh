@@ -288,9 +288,19 @@ __device__ __forceinline__ void weno5_nd(double a, double b, double c, double d,
   num = a0 * q0 + a1 * q1 + a2 * q2;
   den = a0 + a1 + a2;
 }
+// Third-order variant (reading A23): candidates {a,b}, {b,c}, linear weights 1/3, 2/3, smoothness (b-a)^2, (c-b)^2; as
+// numerator and denominator over the common denominator e0 e1 like weno5_nd.
+__device__ __forceinline__ void weno3_nd(double a, double b, double c, double& num, double& den) {
+  const double q0 = 0.5 * (3.0 * b - a), q1 = 0.5 * (b + c);
+  const double t0 = b - a, t1 = c - b;
+  const double e0 = 1e-6 + t0 * t0, e1 = 1e-6 + t1 * t1;
+  const double w0 = (1.0 / 3.0) * (e1 * e1), w1 = (2.0 / 3.0) * (e0 * e0);
+  num = w0 * q0 + w1 * q1;
+  den = w0 + w1;
+}
 
 // dF = F_weno - F_central at the interface between node (i,j,k) and its upper neighbour along D (S5, S6)
-template <int D>
+template <int D, int ORD>
 __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, int j, int k, double dF[5]) {
   double rho[6], vel[6][3], Hh[6], pp[6], cs[6];
 #pragma unroll
@@ -355,9 +365,11 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
     fc[n][2] = vn * wc[n][2];
     fc[n][3] = vn * wc[n][3];
     fc[n][4] = vn * wc[n][4] + 0.5 * (e + h);
-    al[0] = fmax(al[0], fabs(vn - cs[n]));
-    al[1] = fmax(al[1], fabs(vn));
-    al[4] = fmax(al[4], fabs(vn + cs[n]));
+    if (ORD == 5 || (n >= 1 && n <= 4)) {                // local LF: the nodes the reconstruction reads (A23)
+      al[0] = fmax(al[0], fabs(vn - cs[n]));
+      al[1] = fmax(al[1], fabs(vn));
+      al[4] = fmax(al[4], fabs(vn + cs[n]));
+    }
   }
   al[2] = al[1]; al[3] = al[1];
   // steps 5-6: split and reconstruct
@@ -368,8 +380,13 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
 #pragma unroll
     for (int n = 0; n < 6; ++n) { fp[n] = 0.5 * (fc[n][s] + al[s] * wc[n][s]); fm[n] = 0.5 * (fc[n][s] - al[s] * wc[n][s]); }
     double np_, dp_, nm_, dm_;
-    weno5_nd(fp[0], fp[1], fp[2], fp[3], fp[4], np_, dp_);
-    weno5_nd(fm[5], fm[4], fm[3], fm[2], fm[1], nm_, dm_);
+    if (ORD == 5) {
+      weno5_nd(fp[0], fp[1], fp[2], fp[3], fp[4], np_, dp_);
+      weno5_nd(fm[5], fm[4], fm[3], fm[2], fm[1], nm_, dm_);
+    } else {
+      weno3_nd(fp[1], fp[2], fp[3], np_, dp_);
+      weno3_nd(fm[4], fm[3], fm[2], nm_, dm_);
+    }
     // range: den ~ (eps + beta)^4 with beta ~ F^2 (F = characteristic flux), so d+ d- ~ F^16 between 1e-48 (smooth
     // data, eps^8) and fp64 overflow at F ~ 1e19: no rescaling needed in any sensible unit system
     fh[s] = (np_ * dm_ + nm_ * dp_) / (dp_ * dm_);
@@ -389,7 +406,7 @@ __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, i
 
 // one thread per listed interface of direction D: dF of the interface above node o -> dFbuf[D][v][o]
 // (IFACE_BELOW entries: the interface below the first node -> dFb, the boundary-plane scratch)
-template <int D, int MB>
+template <int D, int MB, int ORD>
 __global__ void __launch_bounds__(128, MB) k_weno_flux(const __grid_constant__ DevP P, const double* __restrict__ w, const unsigned int* __restrict__ ilist,
                                                    size_t istride, const DevScal* __restrict__ sc, double* __restrict__ dFbuf, double* __restrict__ dFb) {
   const unsigned int n = sc->icount[D];
@@ -401,7 +418,7 @@ __global__ void __launch_bounds__(128, MB) k_weno_flux(const __grid_constant__ D
     const unsigned int o = en & ~IFACE_BELOW, row = o / (unsigned int)P.nx;
     const int i = (int)(o - row * (unsigned int)P.nx), k = (int)(row / (unsigned int)P.ny), j = (int)(row - (unsigned int)k * (unsigned int)P.ny);
     double dF[5];
-    weno_delta<D>(P, w, i - (below && D == 0), j - (below && D == 1), k - (below && D == 2), dF);
+    weno_delta<D, ORD>(P, w, i - (below && D == 0), j - (below && D == 1), k - (below && D == 2), dF);
     if (below) {
       double* ob = dFb + plane_base<D>(P) + plane_index<D>(P, i, j, k);
 #pragma unroll

@@ -126,6 +126,7 @@ const char* validate(const streams_grid* g, const streams_params* p) {
   if (p->order != 2 && p->order != 4 && p->order != 6) return "order must be 2, 4 or 6";
   if (p->weno_enable && (long long)g->nx * g->ny * g->nz > 0x7fffffffLL) return "more than 2^31 nodes with the hybrid switch on (interface lists)";
   if (p->weno_enable && !(p->sensor_eps > 0.0)) return "sensor_eps must be > 0 (Eq. 8 is 0/0 in uniform flow otherwise)";
+  if (p->weno_order != 0 && p->weno_order != 3 && p->weno_order != 5) return "weno_order must be 3 or 5 (0 = 5)";
   if (p->visc_model != STREAMS_VISC_POWER && p->visc_model != STREAMS_VISC_SUTHERLAND) return "unknown visc_model";
   if (!(p->cfl > 0.0) && !(p->dt_fixed > 0.0)) return "cfl > 0 or dt_fixed > 0 required";
   const int n[3] = {g->nx, g->ny, g->nz};
@@ -639,12 +640,21 @@ static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, d
   if ((rc = run_list(c))) return rc;
   // 128 registers (4 CTAs of 128 threads per SM, 224 B of spills): 16 warps hide the fp64 latency of the reconstructions
   // better than 232 registers at 8 warps (config 4, ms per RK3 step: 22.9 / 20.5 / 20.4 with 2 / 3 / 4 CTAs per SM)
-  k_weno_flux<0, 4><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
-  LAUNCH_CHECK("k_weno_flux<0>");
-  k_weno_flux<1, 4><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
-  LAUNCH_CHECK("k_weno_flux<1>");
-  k_weno_flux<2, 4><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
-  LAUNCH_CHECK("k_weno_flux<2>");
+  if (c->p.weno_order == 3) {      // third-order variant (include/streams.h, weno_order): same lists, same launch shape
+    k_weno_flux<0, 4, 3><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    LAUNCH_CHECK("k_weno_flux<0,3>");
+    k_weno_flux<1, 4, 3><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    LAUNCH_CHECK("k_weno_flux<1,3>");
+    k_weno_flux<2, 4, 3><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    LAUNCH_CHECK("k_weno_flux<2,3>");
+  } else {
+    k_weno_flux<0, 4, 5><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    LAUNCH_CHECK("k_weno_flux<0>");
+    k_weno_flux<1, 4, 5><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    LAUNCH_CHECK("k_weno_flux<1>");
+    k_weno_flux<2, 4, 5><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    LAUNCH_CHECK("k_weno_flux<2>");
+  }
   k_weno_apply<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->dFbuf, c->dFb, R, q_new, beta);
   LAUNCH_CHECK("k_weno_apply");
   return STREAMS_OK;

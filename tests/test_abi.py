@@ -38,6 +38,7 @@ def test_struct_layout_matches_c(blib):
 int main(void){
   printf("%zu %zu %zu\n", sizeof(streams_grid), sizeof(streams_params), sizeof(streams_diag));
   printf("%zu %zu %zu %zu\n", offsetof(streams_params, visc_model), offsetof(streams_params, bc), offsetof(streams_params, fs), offsetof(streams_params, dt_fixed));
+  printf("%zu\n", offsetof(streams_params, weno_order));
   printf("%zu %zu %zu\n", offsetof(streams_diag, weno_ifaces), offsetof(streams_diag, nonfinite), offsetof(streams_diag, max_speed));
   return 0; }'''
     with tempfile.TemporaryDirectory() as td:
@@ -50,7 +51,8 @@ int main(void){
     P, D = blib.StreamsParams, blib.StreamsDiag
     assert vals[:3] == [C.sizeof(blib.StreamsGrid), C.sizeof(P), C.sizeof(D)]
     assert vals[3:7] == [P.visc_model.offset, P.bc.offset, P.fs.offset, P.dt_fixed.offset]
-    assert vals[7:10] == [D.weno_ifaces.offset, D.nonfinite.offset, D.max_speed.offset]
+    assert vals[7] == P.weno_order.offset
+    assert vals[8:11] == [D.weno_ifaces.offset, D.nonfinite.offset, D.max_speed.offset]
 
 
 def test_workspace_and_validation(blib):
@@ -67,6 +69,8 @@ def test_workspace_and_validation(blib):
     assert blib.workspace_bytes(wl.grid, bad) == 0
     bad = dict(wl.params, weno_enable=1, sensor_eps=0.0)
     assert blib.workspace_bytes(wl.grid, bad) == 0
+    assert blib.workspace_bytes(wl.grid, dict(wl.params, weno_order=7)) == 0
+    assert blib.workspace_bytes(wl.grid, dict(wl.params, weno_order=3)) == blib.workspace_bytes(wl.grid, dict(wl.params, weno_order=0)) > 0
     # create without a workspace fails with ENOMEM before any CUDA call
     g, p = blib.make_grid(wl.grid), blib.make_params(wl.params)
     import numpy as np

@@ -161,6 +161,9 @@ SMALL = {
     "sutherland": lambda: W.random_periodic(24, 12, 10, params=P(visc_model=W.VISC_SUTHERLAND)),
     "weno_mixed": lambda: W.random_periodic(40, 20, 12, params=P(weno_enable=1, sensor_threshold=0.3, sensor_eps=0.1)),
     "weno_everywhere": lambda: W.random_periodic(20, 12, 10, params=P(weno_enable=1, sensor_threshold=-1.0, sensor_eps=0.1)),
+    # the WENO order as a parameter (k_weno_flux<D, MB, 3>; reading A23)
+    "weno3_mixed": lambda: W.random_periodic(40, 20, 12, params=P(weno_enable=1, sensor_threshold=0.3, sensor_eps=0.1, weno_order=3)),
+    "weno3_everywhere": lambda: W.random_periodic(20, 12, 10, params=P(weno_enable=1, sensor_threshold=-1.0, sensor_eps=0.1, weno_order=3)),
     "tiny_4x4x4": lambda: W.random_periodic(4, 4, 4, params=P()),
     "line_x": lambda: W.random_periodic(50, 1, 1, params=P()),
     "line_y": lambda: W.random_periodic(1, 50, 1, params=P()),
@@ -171,6 +174,7 @@ SMALL = {
     "sbli_ragged": lambda: W.config4_sbli(45, 30, 7, Lx=10.0),
     # every interface WENO with non-periodic x and y: the interface lists hold N + a boundary plane of entries
     "sbli_weno_everywhere": lambda: mod(W.config4_sbli(45, 30, 7, Lx=10.0), sensor_threshold=-1.0),
+    "sbli_weno3_everywhere": lambda: mod(W.config4_sbli(45, 30, 7, Lx=10.0), sensor_threshold=-1.0, weno_order=3),
     # forcing and the hybrid switch together (unfused fallback: k_rhs<0>, WENO correction, k_update)
     "channel_weno_forcing": lambda: mod(W.config3_channel(37, 19, 11), weno_enable=1, sensor_threshold=0.2, sensor_eps=0.1),
     # forcing with Dirichlet wall nodes (lazy forcing must leave the overridden wall rows alone)
@@ -183,7 +187,7 @@ SMALL = {
     "boundary_layer_weno": lambda: mod(W.config7_boundary_layer(45, 30, 7, Lx=10.0), weno_enable=1, sensor_threshold=-1.0),
 }
 
-STEPPED = ["boundary_layer_small", "boundary_layer_weno", "channel_paper_small", "channel_ragged", "channel_weno_forcing", "channel_node_walls", "sbli_weno_everywhere", "weno_mixed", "several_tiles_and_chunks"]
+STEPPED = ["boundary_layer_small", "boundary_layer_weno", "channel_paper_small", "channel_ragged", "channel_weno_forcing", "channel_node_walls", "sbli_weno_everywhere", "sbli_weno3_everywhere", "weno_mixed", "weno3_mixed", "several_tiles_and_chunks"]
 
 
 @pytest.mark.parametrize("name", list(SMALL))

@@ -248,16 +248,17 @@ def test_nccl_self_exchange_world_size_one(env, case):
     one.close()
 
 
-@pytest.mark.parametrize("case", ["weno_box", "sbli"])
+@pytest.mark.parametrize("case", ["weno_box", "weno3_box", "sbli"])
 def test_hybrid_switch_on_slabs_is_bitwise_the_undivided_run(env, case):
     """The hybrid switch across slab faces: the node-flag words of the neighbour's three planes are
     swapped between stage_rhs and stage_end; the interfaces next to a face are then flagged, listed and corrected exactly as
     in the undivided run.  `sbli` adds the frozen inflow (captured with its ghost planes after the first halo swap), the
     node wall, the shock generator and the characteristic outflow."""
     torch, binding, slab, ob = env
-    if case == "weno_box":
+    if case in ("weno_box", "weno3_box"):
         wl = W.random_periodic(32, 16, 36, params=W.default_params(Rgas=1 / 1.4, mu_ref=5e-3, weno_enable=1,
-                                                                   sensor_threshold=0.3, sensor_eps=0.1))
+                                                                   sensor_threshold=0.3, sensor_eps=0.1,
+                                                                   weno_order=3 if case == "weno3_box" else 5))
         nsl = 3
     else:
         wl = W.config4_sbli(64, 40, 16)
