@@ -185,10 +185,17 @@ int streams_step(streams_ctx* ctx, int nsteps);
  * `part`: STREAMS_PART_ALL launches the whole grid.  For overlap, STREAMS_PART_INTERIOR launches the z-chunks that read
  * no ghost plane (possibly none on a thin slab) and may run while the halos are in flight; STREAMS_PART_BOUNDARY then
  * launches the first and the last chunk and the reductions.  Calls out of this order return STREAMS_ESTATE.
- * streams_step refuses a context with a BC_HALO face.  All calls are asynchronous on the context stream. */
+ * streams_step refuses a context with a BC_HALO face.  All calls are asynchronous on the context stream.
+ * forcing = 1 TOGETHER WITH weno_enable = 1: the body force is the sum of the residual AFTER its WENO correction
+ * (PAPER.md:57, 77-79), and on a slab that correction needs the neighbours' flag words.  The stage is then
+ *         streams_stage_rhs | [caller: swap the flag words] | streams_stage_mid(stage): WENO correction of R, sums ->
+ *         red[0], red[1] | [caller: SUM of red[0..1]] | streams_stage_end(stage): f, Eq. 11.
+ * streams_stage_mid is optional on a context without a BC_HALO face (streams_stage_end then does its work) and does
+ * nothing for other parameter combinations; at most once per stage, else STREAMS_ESTATE. */
 enum { STREAMS_PART_ALL = 0, STREAMS_PART_INTERIOR = 1, STREAMS_PART_BOUNDARY = 2 };
 int streams_step_begin(streams_ctx* ctx);
 int streams_stage_rhs(streams_ctx* ctx, int stage, int part);
+int streams_stage_mid(streams_ctx* ctx, int stage);
 int streams_stage_end(streams_ctx* ctx, int stage);
 
 /* DEVICE pointer (inside the caller's workspace, valid for the life of the context) to four doubles:

@@ -16,7 +16,7 @@ STREAMS_OK, STREAMS_EINVAL, STREAMS_ECUDA, STREAMS_ENOMEM, STREAMS_ENONFINITE, S
 
 EXPORTS = ["streams_workspace_bytes", "streams_create", "streams_set_state", "streams_set_state_host",
            "streams_get_state", "streams_get_state_host", "streams_rhs", "streams_sensor", "streams_step",
-           "streams_diagnostics", "streams_step_begin", "streams_stage_rhs", "streams_stage_end", "streams_reduce_ptr",
+           "streams_diagnostics", "streams_step_begin", "streams_stage_rhs", "streams_stage_mid", "streams_stage_end", "streams_reduce_ptr",
            "streams_halo_bytes", "streams_halo_pack", "streams_halo_unpack", "streams_flag_halo_bytes", "streams_flag_halo_pack",
            "streams_flag_halo_unpack", "streams_stats_accumulate", "streams_stats_read", "streams_stats_reset", "streams_profile", "streams_profile_read", "streams_fp64_peak", "streams_max_speed_static",
            "streams_launch_count", "streams_last_error", "streams_destroy"]
@@ -78,6 +78,7 @@ def lib():
         L.streams_step_begin.argtypes = [C.c_void_p]
         L.streams_stage_rhs.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.streams_stage_end.argtypes = [C.c_void_p, C.c_int]
+        L.streams_stage_mid.argtypes = [C.c_void_p, C.c_int]
         L.streams_reduce_ptr.argtypes = [C.c_void_p]
         L.streams_reduce_ptr.restype = C.c_void_p
         L.streams_halo_bytes.argtypes = [C.c_void_p]
@@ -285,6 +286,10 @@ class Streams:
 
     def stage_rhs(self, stage, part=0):
         self._chk(lib().streams_stage_rhs(self._h, int(stage), int(part)))
+
+    def stage_mid(self, stage):
+        """forcing with the hybrid switch: WENO correction of R and its sums -> red[0..1] (after the flag-word swap)."""
+        self._chk(lib().streams_stage_mid(self._h, int(stage)))
 
     def stage_end(self, stage):
         self._chk(lib().streams_stage_end(self._h, int(stage)))

@@ -58,6 +58,7 @@ struct streams_ctx {
   int stage_half;                      // streams_stage_end comes next (half: 0 = rhs pending, 1 = end pending)
   int inflow_pending;                  // z-slab with INFLOW_FROZEN: the frozen plane is captured once the ghost planes are in
   int parts_done;                      // bit 0: interior chunks launched, bit 1: boundary chunks launched (this stage)
+  int mid_done;                        // forcing + hybrid switch: streams_stage_mid has corrected R and summed it (this stage)
   // TMA descriptors, 4-D (x, y, z, field): per state buffer the tile box (halo 3) and the own-node box (no halo)
   CUtensorMap tmap[2], tmap_own[2];
   int use_tma;                   // 0 when nx is odd (TMA needs 16-byte row strides): tiles are filled by index
@@ -147,9 +148,6 @@ const char* validate(const streams_grid* g, const streams_params* p) {
     }
   }
   if (p->forcing && p->bc[0] != STREAMS_BC_PERIODIC) return "bulk forcing needs a periodic x direction";
-  if (p->bc[4] == STREAMS_BC_HALO || p->bc[5] == STREAMS_BC_HALO) {
-    if (p->weno_enable && p->forcing) return "z-slabs: forcing and the hybrid switch together are not supported";
-  }
   return nullptr;
 }
 
@@ -556,7 +554,7 @@ static int after_set_state(streams_ctx* c, const double* d_w) {
   CK(cudaMemsetAsync(&c->sc->force, 0, sizeof(double), c->st));
   CK(cudaMemsetAsync(&c->sc->time, 0, sizeof(double), c->st));
   if (!(c->p.dt_fixed > 0.0)) CK(cudaMemsetAsync(&c->sc->dt, 0, sizeof(double), c->st));
-  c->has_state = 1; c->step = 0; c->scur = 0; c->dt_ready = 0; c->stage_next = -1; c->stage_half = 0; c->parts_done = 0;
+  c->has_state = 1; c->step = 0; c->scur = 0; c->dt_ready = 0; c->stage_next = -1; c->stage_half = 0; c->parts_done = 0; c->mid_done = 0;
   return STREAMS_OK;
 }
 
@@ -792,6 +790,19 @@ static int do_stage_rhs(streams_ctx* c, int l, int part, bool single) {
   return STREAMS_OK;
 }
 
+// forcing with the hybrid switch, between the halves: the body force needs the sum of the CORRECTED R, and on z-slabs the
+// correction needs the neighbours' flag words, which the caller swaps after do_stage_rhs: WENO correction of R, then the
+// partial sums into red[0..1] (not taken: the caller combines them across the slabs before do_stage_end)
+static int do_stage_mid(streams_ctx* c) {
+  if (!(c->p.forcing && c->p.weno_enable)) return STREAMS_OK;
+  int rc;
+  double* Sc = c->S[c->scur ^ 1];
+  if ((rc = run_weno(c, c->qbuf[c->cur], Sc, nullptr, 0.0))) return rc;
+  if ((rc = force_from_partials(c, Sc, false, false))) return rc;
+  c->mid_done = 1;
+  return STREAMS_OK;
+}
+
 // second half of RK stage l: f = -red[0] / red[1] (combined across z-slabs by the caller), the forcing fix, the WENO
 // correction; after the last stage the CFL maximum of the new state and the time
 static int do_stage_end(streams_ctx* c, int l, bool single) {
@@ -813,8 +824,14 @@ static int do_stage_end(streams_ctx* c, int l, bool single) {
   } else if (c->p.forcing) {
     double* Sp = c->S[c->scur];
     double* Sc = c->S[c->scur ^ 1];
-    if (c->p.weno_enable && (rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
-    if ((rc = force_from_partials(c, Sc, !c->p.weno_enable, true))) return rc;
+    if (c->mid_done) {
+      // streams_stage_mid has corrected R and left its sums in red[0..1]; the caller has combined them across the slabs
+      k_force_take<<<1, 1, 0, c->st>>>(c->sc);
+      LAUNCH_CHECK("k_force_take");
+    } else {
+      if (c->p.weno_enable && (rc = run_weno(c, w, Sc, nullptr, 0.0))) return rc;
+      if ((rc = force_from_partials(c, Sc, !c->p.weno_enable, true))) return rc;
+    }
     k_update<<<rg, RT, 0, c->st>>>(c->P, w, Sp, Sc, c->sc, RK_ALPHA[l], RK_BETA[l], 1, l < 2 ? 1 : 0);
     LAUNCH_CHECK("k_update");
     c->scur ^= 1;
@@ -895,7 +912,7 @@ int streams_step_begin(streams_ctx* c) {
   if (c->stage_next >= 0) return fail(c, STREAMS_ESTATE, "streams_step_begin: the previous staged step is not finished");
   const int rc = do_step_begin(c);
   if (rc) return rc;
-  c->stage_next = 0; c->stage_half = 0; c->parts_done = 0;
+  c->stage_next = 0; c->stage_half = 0; c->parts_done = 0; c->mid_done = 0;
   return STREAMS_OK;
 }
 
@@ -917,13 +934,22 @@ int streams_stage_rhs(streams_ctx* c, int stage, int part) {
   return STREAMS_OK;
 }
 
+int streams_stage_mid(streams_ctx* c, int stage) {
+  if (!c) return fail(c, STREAMS_EINVAL, "null argument");
+  DevGuard dg(c->device);
+  if (c->stage_next != stage || c->stage_half != 1 || c->mid_done) return fail(c, STREAMS_ESTATE, "streams_stage_mid out of order (once, between streams_stage_rhs and streams_stage_end)");
+  return do_stage_mid(c);
+}
+
 int streams_stage_end(streams_ctx* c, int stage) {
   if (!c) return fail(c, STREAMS_EINVAL, "null argument");
   DevGuard dg(c->device);
   if (c->stage_next != stage || c->stage_half != 1) return fail(c, STREAMS_ESTATE, "streams_stage_end out of order");
+  if (c->zpad && c->p.forcing && c->p.weno_enable && !c->mid_done)
+    return fail(c, STREAMS_ESTATE, "streams_stage_end: a z-slab with forcing and the hybrid switch needs streams_stage_mid first");
   const int rc = do_stage_end(c, stage, false);
   if (rc) return rc;
-  c->stage_half = 0; c->parts_done = 0;
+  c->stage_half = 0; c->parts_done = 0; c->mid_done = 0;
   if (stage == 2) { c->stage_next = -1; c->step++; } else c->stage_next = stage + 1;
   return STREAMS_OK;
 }

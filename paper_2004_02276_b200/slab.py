@@ -4,7 +4,8 @@ Host-side orchestration only.  Every slab is one context of the CUDA library who
 `BC_HALO`; all arithmetic runs in the library's kernels through the staged C-ABI calls (include/streams.h):
 
     step_begin | MAX of red[2] | for each stage: swap halos, stage_rhs(interior) while the swap is in flight,
-    stage_rhs(boundary), SUM of red[0..1] (forcing), swap of the node-flag words (hybrid switch), stage_end.
+    stage_rhs(boundary), SUM of red[0..1] (forcing), swap of the node-flag words (hybrid switch), stage_end
+    (forcing AND hybrid switch: flag swap, stage_mid, SUM, stage_end).
 
 The messages move by `torch.distributed` point-to-point operations between processes (NCCL on GPUs, one process per
 GPU) and by device-to-device copies between slabs of the same process.
@@ -297,10 +298,18 @@ class SlabGroup:
                 for i, s in enumerate(sl):
                     sy[i].main_wait(halo_ready[i])
                     s.stage_rhs(stage, PART_BOUNDARY if self.overlap else PART_ALL)
-                if self.forcing and self.combine:
-                    self.reducer.sum(sl, sy)
-                if self.weno:
+                if self.forcing and self.weno:
+                    # the body force is the sum of the residual AFTER its WENO correction, which needs the neighbours' flags
                     self.swap_flags()
+                    for s in sl:
+                        s.stage_mid(stage)
+                    if self.combine:
+                        self.reducer.sum(sl, sy)
+                else:
+                    if self.forcing and self.combine:
+                        self.reducer.sum(sl, sy)
+                    if self.weno:
+                        self.swap_flags()
                 for s in sl:
                     s.stage_end(stage)
 

@@ -185,6 +185,80 @@ def test_channel_slabs_with_forcing(env):
     o.close()
 
 
+def test_channel_slabs_with_forcing_and_the_hybrid_switch(env):
+    """forcing = 1 with weno_enable = 1 on slabs: the body force is the sum of the residual after its
+    WENO correction, which needs the neighbours' flag words: stage_rhs | flag swap | stage_mid | SUM | stage_end.
+    (1) fed: the undivided context runs the same staged calls in lockstep and its red[0..1] go to every slab -> bitwise,
+    and equal to streams_step; (2) combined: the slabs' sums are added -> summation-order round-off; oracle parity."""
+    import dataclasses
+    torch, binding, slab, ob = env
+    wl = W.config3_channel(64, 32, 40)
+    wl = dataclasses.replace(wl, params=dict(wl.params, weno_enable=1, sensor_threshold=0.2, sensor_eps=0.1))
+    w0 = wl.state()
+    nsl, nsteps = 2, 3
+    one = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    one.set_state(torch.from_numpy(w0).cuda())
+    ctxs, specs, _ = make_slabs(env, wl, nsl)
+    grp = slab.SlabGroup(ctxs, nsl, periodic=True, reducer=HostReducer(torch), forcing=True, weno=True)
+
+    def feed(lo, hi):
+        one.stream.synchronize()
+        v = one.red[lo:hi].clone()
+        for c in ctxs:
+            with torch.cuda.stream(c.stream):
+                c.red[lo:hi].copy_(v)
+            c.stream.synchronize()
+
+    for _ in range(nsteps):
+        one.step_begin()
+        for c in ctxs:
+            c.step_begin()
+        feed(2, 3)
+        for stage in range(3):
+            ready = grp.swap_halos()
+            one.stage_rhs(stage, one.PART_ALL)
+            for i, c in enumerate(ctxs):
+                grp.syncs[i].main_wait(ready[i])
+                c.stage_rhs(stage, c.PART_INTERIOR)
+                c.stage_rhs(stage, c.PART_BOUNDARY)
+            if stage == 0:
+                with pytest.raises(binding.StreamsError):          # a slab cannot sum before the flags are in
+                    ctxs[0].stage_end(stage)
+            grp.swap_flags()
+            one.stage_mid(stage)
+            for c in ctxs:
+                c.stage_mid(stage)
+            feed(0, 2)
+            one.stage_end(stage)
+            for c in ctxs:
+                c.stage_end(stage)
+    ref = one.get_state().cpu().numpy()
+    assert sum(one.diagnostics().weno_ifaces) > 0, "the case must exercise the WENO branch"
+    got = gather(ctxs)
+    assert np.array_equal(got, ref), np.abs(got - ref).max()
+    two = binding.Streams(wl.grid, wl.x, wl.y, wl.z, wl.params)    # streams_step = the staged calls without stage_mid
+    two.set_state(torch.from_numpy(w0).cuda())
+    two.step(nsteps)
+    assert np.array_equal(two.get_state().cpu().numpy(), ref)
+    with pytest.raises(binding.StreamsError):
+        two.stage_mid(0)                                           # no staged step is open
+    # (2) combined
+    ctxs2, _, _ = make_slabs(env, wl, nsl)
+    grp2 = slab.SlabGroup(ctxs2, nsl, periodic=True, reducer=HostReducer(torch), forcing=True, weno=True)
+    grp2.step(nsteps)
+    got2 = gather(ctxs2)
+    assert l2(got2, ref) < 1e-13
+    f1, f2 = one.diagnostics().forcing, ctxs2[0].diagnostics().forcing
+    assert abs(f1 - f2) <= 1e-12 * abs(f1)
+    o = ob.Oracle(wl.grid, wl.x, wl.y, wl.z, wl.params)
+    o.set_state(w0)
+    o.step(nsteps)
+    assert l2(got2, o.get_state()) < STEP_TOL
+    for c in ctxs + ctxs2 + [one, two]:
+        c.close()
+    o.close()
+
+
 def test_staged_calls_enforce_their_order(env):
     torch, binding, slab, _ = env
     wl = W.random_periodic(32, 16, 16, params=W.default_params(Rgas=1 / 1.4, mu_ref=5e-3))

@@ -201,3 +201,121 @@ def test_two_gloo_ranks_exchange_and_reduce(periodic):
     for rank, err, sent in res:
         assert err < 1e-13, (rank, err)
         assert sent == 2 * 3 * (2 if periodic else 1)
+
+
+# ---- forcing together with the hybrid switch: flag swap | stage_mid | SUM | stage_end (include/streams.h) --------------
+class ToyFlagSlab(ToySlab):
+    """The toy with node flags (r > 0 of field 0) whose neighbours' values enter a correction of r (a 7-plane window
+    of flags, like the interface flags of the hybrid switch) BEFORE r is summed: the sum left by stage_rhs is poison."""
+
+    def flag_shape(self):
+        return (3, NY, NX)
+
+    def new_flag_buffer(self):
+        return torch.full(self.flag_shape(), -7, dtype=torch.int32)
+
+    def stage_rhs(self, stage, part):
+        super().stage_rhs(stage, part)
+        if part == slab.PART_INTERIOR:
+            return
+        self.flag = (self.r[0] > 0).astype(np.int32) * (1 + np.arange(self.nz)[:, None, None] % 3)
+        self.fl = [None, None]
+        self.red[0] = float("nan")                  # only stage_mid knows the sum
+        self.mid = False
+
+    def flag_halo_pack(self, face, out, stream=None):
+        out.copy_(torch.from_numpy(np.ascontiguousarray(self.flag[:3] if face == slab.FACE_ZMIN else self.flag[-3:])))
+        self.log.append(("fpack", face))
+
+    def flag_halo_unpack(self, face, buf, stream=None):
+        self.fl[0 if face == slab.FACE_ZMIN else 1] = buf.numpy().copy()
+        self.log.append(("funpack", face))
+
+    def stage_mid(self, stage):
+        lo = self.fl[0] if self.has[0] else np.repeat(self.flag[:1], 3, axis=0)
+        hi = self.fl[1] if self.has[1] else np.repeat(self.flag[-1:], 3, axis=0)
+        assert lo is not None and hi is not None and (lo >= 0).all() and (hi >= 0).all(), "flag words were not in place"
+        ext = np.concatenate([lo, self.flag, hi], axis=0)
+        self.r = self.r + 0.01 * sum((m + 1) * ext[m:m + self.nz] for m in range(7))[None]
+        self.red[0] = float(self.r[0].sum())
+        self.red[1] = float(self.r[0].size)
+        self.mid = True
+        self.log.append(("mid", stage))
+
+    def stage_end(self, stage):
+        assert self.mid, "stage_end before stage_mid"
+        super().stage_end(stage)
+
+
+def toy_flag_reference(q, periodic, nsteps):
+    q = q.copy()
+    nz = q.shape[1]
+    for _ in range(nsteps):
+        dt = 0.1 / np.abs(q).max()
+        for stage in range(3):
+            pad = (lambda a: np.concatenate([a[-3:], a, a[:3]], axis=0)) if periodic else \
+                  (lambda a: np.concatenate([a[:1]] * 3 + [a] + [a[-1:]] * 3, axis=0))
+            ext = np.stack([pad(q[v]) for v in range(7)])
+            r = sum(COEF[m] * ext[:, m:m + nz] for m in range(7))
+            # the flag multiplier is the plane index inside the OWNING slab; the test cuts nz into equal slabs of `per` planes
+            flag = (r[0] > 0).astype(np.int32) * (1 + (np.arange(nz) % toy_flag_reference.per)[:, None, None] % 3)
+            fe = pad(flag)
+            r = r + 0.01 * sum((m + 1) * fe[m:m + nz] for m in range(7))[None]
+            q = q + dt * (stage + 1) * (r - r[0].sum() / r[0].size)
+    return q
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+def test_three_local_slabs_with_flags_and_forcing(periodic):
+    nz, nsl = 30, 3
+    toy_flag_reference.per = nz // nsl
+    q0 = field(nz, seed=5) - 1.0                   # both signs: the flags are not all equal
+    slabs = []
+    for i in range(nsl):
+        k0, k1 = slab.slab_range(nz, nsl, i)
+        lo, hi = slab.neighbours(i, nsl, periodic)
+        slabs.append(ToyFlagSlab(q0[:, k0:k1], lo, hi))
+    grp = slab.SlabGroup(slabs, nsl, periodic=periodic, reducer=LocalReducer(), syncs=[slab.NoSync() for _ in slabs],
+                         forcing=True, cfl_dt=True, overlap=True, weno=True)
+    grp.step(2)
+    got = np.concatenate([s.interior() for s in slabs], axis=1)
+    ref = toy_flag_reference(q0, periodic, 2)
+    assert np.abs(got - ref).max() < 1e-13
+    names = [e[0] for e in slabs[1].log[1:13]]      # first stage of the middle slab
+    assert names == ["pack", "pack", "unpack", "unpack", "rhs", "rhs", "fpack", "fpack", "funpack", "funpack", "mid", "end"]
+
+
+def _flag_worker(rank, world, port, periodic, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    nz = 16
+    toy_flag_reference.per = nz // world
+    q0 = field(nz, seed=13) - 1.0
+    k0, k1 = slab.slab_range(nz, world, rank)
+    lo, hi = slab.neighbours(rank, world, periodic)
+    s = ToyFlagSlab(q0[:, k0:k1], lo, hi)
+    grp = slab.SlabGroup([s], world, rank=rank, periodic=periodic, dist=dist, syncs=[slab.NoSync()], forcing=True, cfl_dt=True,
+                         weno=True)
+    grp.step(2)
+    ref = toy_flag_reference(q0, periodic, 2)[:, k0:k1]
+    q.put((rank, float(np.abs(s.interior() - ref).max()), grp.messages_sent))
+    dist.destroy_process_group()
+
+
+def test_two_gloo_ranks_with_flags_and_forcing():
+    sk = socket.socket()
+    sk.bind(("127.0.0.1", 0))
+    port = sk.getsockname()[1]
+    sk.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_flag_worker, args=(r, 2, port, True, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, err, sent in res:
+        assert err < 1e-13, (rank, err)
+        assert sent == 2 * 3 * 2 * 2                # halos and flag words: two messages each per stage
