@@ -223,7 +223,7 @@ int streams_halo_unpack(streams_ctx* ctx, int face, const double* d_buf, void* c
  * the same way as the state halos: message [3][ny][ceil(nx/32)] 32-bit words = streams_flag_halo_bytes() bytes (0 when
  * the switch is off).  With a frozen inflow the slab captures the inflow plane (its ghost planes included) at the first
  * use of the state after streams_set_state, i.e. after the caller's first halo swap.  streams_rhs refuses a slab with the
- * hybrid switch (one call cannot contain the swap); streams_sensor and the interface counts of streams_diagnostics on a
+ * hybrid switch (one call cannot contain the swap) and a slab with forcing (the body force is a sum over all slabs); streams_sensor and the interface counts of streams_diagnostics on a
  * slab use the ghost flag words of the last stage. */
 size_t streams_flag_halo_bytes(const streams_ctx* ctx);
 int streams_flag_halo_pack(streams_ctx* ctx, int face, unsigned int* d_buf, void* cuda_stream);

@@ -299,15 +299,43 @@ __device__ __forceinline__ void weno3_nd(double a, double b, double c, double& n
   den = w0 + w1;
 }
 
+// rho, u, v, w, T of a (possibly ghost) node by the rules of S1, out of line and returned by value (stays in registers)
+struct P5 { double rho, u, v, w, T; };
+__device__ __noinline__ P5 fetch_prim5_ghost(const DevP& P, const double* __restrict__ w, int i, int j, int k) {
+  Prim q;
+  fetch_prim5(P, w, i, j, k, q);
+  P5 r;
+  r.rho = q.rho; r.u = q.u; r.v = q.v; r.w = q.w; r.T = q.T;
+  return r;
+}
+
 // dF = F_weno - F_central at the interface between node (i,j,k) and its upper neighbour along D (S5, S6)
 template <int D, int ORD>
 __device__ void weno_delta(const DevP& P, const double* __restrict__ w, int i, int j, int k, double dF[5]) {
   double rho[6], vel[6][3], Hh[6], pp[6], cs[6];
+  // The six stencil nodes i-2 .. i+3 along D.  Nearly every listed interface has all six inside the grid: plain strided
+  // loads.  The ghost rules of S1 (index maps, reflection, inflow / free-stream sources) cost ~150 instructions per node
+  // when inlined six times (the kernel was 3700 instructions, 60 KB: `no_instruction` was its second largest stall);
+  // stencils that reach a face take them through ONE out-of-line copy.
+  // A periodic direction only wraps the index and a BC_HALO face stores its ghost planes around the state: both stay
+  // on the plain path (all of config 2; a warp whose lanes disagree pays both paths).
+  const int id = D == 0 ? i : (D == 1 ? j : k), nd = D == 0 ? P.nx : (D == 1 ? P.ny : P.nz);
+  const bool per = P.bc[2 * D] == BC_PERIODIC;
+  const bool inside = (id >= 2 || per || (D == 2 && P.bc[4] == BC_HALO)) && (id + 3 < nd || per || (D == 2 && P.bc[5] == BC_HALO));
+  const long long st = D == 0 ? 1 : (D == 1 ? (long long)P.nx : P.nxy);
+  const double* q0 = w + (((long long)k * P.ny + j) * P.nx + i) - id * st;      // index 0 along D
 #pragma unroll
   for (int n = 0; n < 6; ++n) {
-    const int off = n - 2;
-    Prim q;
-    fetch_prim5(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0), q);
+    P5 q;
+    if (inside) {
+      int m = id + n - 2;
+      if (per) m = m < 0 ? m + nd : (m >= nd ? m - nd : m);
+      const double* qn = q0 + m * st;
+      q.rho = __ldg(qn); q.u = __ldg(qn + P.QS); q.v = __ldg(qn + 2 * P.QS); q.w = __ldg(qn + 3 * P.QS); q.T = __ldg(qn + 4 * P.QS);
+    } else {
+      const int off = n - 2;
+      q = fetch_prim5_ghost(P, w, i + (D == 0 ? off : 0), j + (D == 1 ? off : 0), k + (D == 2 ? off : 0));
+    }
     rho[n] = q.rho; vel[n][0] = q.u; vel[n][1] = q.v; vel[n][2] = q.w;
     derive_pH(P, q.rho, q.u, q.v, q.w, q.T, pp[n], Hh[n]);
     cs[n] = sqrt(P.gam * P.Rgas * q.T);

@@ -693,6 +693,7 @@ int streams_rhs(streams_ctx* c, double* d_rhs) {
   DevGuard dg(c->device);
   if (!c->has_state) return fail(c, STREAMS_ESTATE, "no state set");
   if (c->zpad && c->p.weno_enable) return fail(c, STREAMS_EINVAL, "streams_rhs on a z-slab with the hybrid switch: the flag words are swapped between the staged calls");
+  if (c->zpad && c->p.forcing) return fail(c, STREAMS_EINVAL, "streams_rhs on a z-slab with forcing: the body force is a sum over all slabs, combined between the staged calls");
   const double* w = c->qbuf[c->cur];
   int rc;
   if ((rc = ensure_inflow(c))) return rc;

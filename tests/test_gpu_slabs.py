@@ -275,6 +275,15 @@ def test_staged_calls_enforce_their_order(env):
     with pytest.raises(binding.StreamsError):
         c.stage_rhs(1)                               # wrong stage
     c.close()
+    # streams_rhs is one call: it refuses the slabs whose residual needs an exchange in the middle of it
+    for wl2 in (W.config3_channel(32, 16, 16), W.random_periodic(32, 16, 16, params=W.default_params(
+            Rgas=1 / 1.4, mu_ref=5e-3, weno_enable=1, sensor_threshold=0.3, sensor_eps=0.1))):
+        sp2 = slab.slab_spec(wl2.grid, wl2.z, wl2.params, 2, 0)
+        c2 = binding.Streams(sp2.grid, wl2.x, wl2.y, sp2.z, sp2.params)
+        c2.set_state(torch.from_numpy(np.ascontiguousarray(wl2.state()[:, sp2.k0:sp2.k1])).cuda())
+        with pytest.raises(binding.StreamsError):
+            c2.rhs()                                 # forcing: sum over all slabs; hybrid switch: neighbours' flag words
+        c2.close()
     # a non-periodic direction cannot take BC_HALO outside z
     p = dict(wl.params)
     p["bc"] = [8, 8, 0, 0, 0, 0]
