@@ -20,8 +20,8 @@
  *    hands them to `streams_create`, and keeps them alive until `streams_destroy`.
  *    The context owns only O(nx+ny+nz) metric arrays and a few scalars on the device.
  *    Workspace: two states of 7 stored primitives (112 B/node), two RK registers
- *    (80 B/node), reduction partials; with weno_enable also the sensor field, node and
- *    interface lists and the interface-flux scratch (about 154 B/node more).
+ *    (80 B/node), reduction partials; with weno_enable also the node flags, node and
+ *    interface lists and the interface-flux scratch (about 146 B/node more).
  *  - All kernels are enqueued on the `cuda_stream` given at creation (a cudaStream_t
  *    passed as void*, NULL = legacy default stream).  Only `streams_diagnostics`,
  *    the *_host copies and `streams_destroy` synchronise that stream.

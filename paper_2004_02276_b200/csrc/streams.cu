@@ -226,7 +226,6 @@ Layout make_layout(const streams_grid& g, const streams_params& p) {
   for (int i = 0; i < 2; ++i) L.S[i] = c.take(5 * N * sizeof(double));
   L.theta = L.nflag = L.fbits = L.lmask = L.list = L.ilist = L.dFbuf = L.dFb = 0;
   if (p.weno_enable) {
-    L.theta = c.take(N * sizeof(double));
     L.nflag = c.take(N);
     L.fbits = c.take((size_t)g.ny * (g.nz + 2 * L.zpad) * ((g.nx + 31) / 32) * sizeof(unsigned int));
     L.lmask = c.take(N);
@@ -399,7 +398,7 @@ int streams_create(const streams_grid* g, const double* hx, const double* hy, co
   const size_t zoff = (size_t)L.zpad * g->nx * g->ny;      // qbuf points at the first INTERIOR plane
   for (int i = 0; i < 2; ++i) { c->qbuf[i] = (double*)(base + L.w[i]) + zoff; c->S[i] = (double*)(base + L.S[i]); }
   if (p->weno_enable) {
-    c->theta = (double*)(base + L.theta); c->nflag = (unsigned char*)(base + L.nflag);
+    c->theta = nullptr; c->nflag = (unsigned char*)(base + L.nflag);
     c->fbits = (unsigned int*)(base + L.fbits) + (size_t)L.zpad * g->ny * ((g->nx + 31) / 32); c->lmask = (unsigned char*)(base + L.lmask); c->list = (unsigned int*)(base + L.list);
     c->ilist = (unsigned int*)(base + L.ilist); c->dFbuf = (double*)(base + L.dFbuf); c->dFb = (double*)(base + L.dFb);
   }
