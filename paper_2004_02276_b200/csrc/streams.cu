@@ -635,21 +635,21 @@ static int run_list(streams_ctx* c) {
 static int run_weno(streams_ctx* c, const double* w, double* R, double* q_new, double beta) {
   int rc;
   if ((rc = run_list(c))) return rc;
-  // 128 registers (4 CTAs of 128 threads per SM, 224 B of spills): 16 warps hide the fp64 latency of the reconstructions
-  // better than 232 registers at 8 warps (config 4, ms per RK3 step: 22.9 / 20.5 / 20.4 with 2 / 3 / 4 CTAs per SM)
+  // 3 CTAs of 128 threads per SM (168 registers, no spills, 12 warps): config 4, ms per RK3 step with 2 / 3 / 4 CTAs per SM:
+  // 18.33 / 16.30 / 16.56 (4 CTAs = 128 registers with 120 B of spills; before the plain-load path of weno_delta 4 was as good)
   if (c->p.weno_order == 3) {      // third-order variant (include/streams.h, weno_order): same lists, same launch shape
-    k_weno_flux<0, 4, 3><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    k_weno_flux<0, 3, 3><<<148 * 3, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
     LAUNCH_CHECK("k_weno_flux<0,3>");
-    k_weno_flux<1, 4, 3><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    k_weno_flux<1, 3, 3><<<148 * 3, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
     LAUNCH_CHECK("k_weno_flux<1,3>");
-    k_weno_flux<2, 4, 3><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    k_weno_flux<2, 3, 3><<<148 * 3, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
     LAUNCH_CHECK("k_weno_flux<2,3>");
   } else {
-    k_weno_flux<0, 4, 5><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    k_weno_flux<0, 3, 5><<<148 * 3, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
     LAUNCH_CHECK("k_weno_flux<0>");
-    k_weno_flux<1, 4, 5><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    k_weno_flux<1, 3, 5><<<148 * 3, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
     LAUNCH_CHECK("k_weno_flux<1>");
-    k_weno_flux<2, 4, 5><<<148 * 4, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
+    k_weno_flux<2, 3, 5><<<148 * 3, 128, 0, c->st>>>(c->P, w, c->ilist, c->istride, c->sc, c->dFbuf, c->dFb);
     LAUNCH_CHECK("k_weno_flux<2>");
   }
   k_weno_apply<<<rgrid_for(c->P.N), RT, 0, c->st>>>(c->P, w, c->list, c->lmask, c->sc, c->dFbuf, c->dFb, R, q_new, beta);
